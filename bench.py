@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py -- log-likelihood evaluations per second of the whole hot path (S1..S5) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload (BASELINE.json `metric`): N = 2^20 samples at dt = 5 s, batch 64 precessing walkers
+with the five-mode set on KEPLER1 orbits (configs[2]), TDI-2 A,E,T at Lagrange order 31,
+forward FFT and the noise-weighted inner product against the zero-noise injection of walker 0
+with the configs[3] PSD and band.  One step = one pass of S1..S5 over the batch.  Inputs are
+seeded and synthetic (paper_2501_08261_b200/synth.py).
+
+Prints ONE JSON line (see DESIGN.md section 8 for every key).  With N > 1 GPUs (torchrun) every
+rank runs its own batch of 64 walkers -- walkers are independent, there is no data-path
+collective -- and the value is the aggregate over ranks ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "loglike evals/sec (2^20 samples, dt=5 s, batch 64)"
+UNIT = "evals/s"
+WORKLOAD = "configs[2] precessing batch: B=64, N=2^20, dt=5 s, 5 modes, KEPLER1 orbits, TDI-2 AET order 31, + configs[3] PSD/band log L"
+CONFIG_ID = 3
+ORDER = 31
+
+# Algorithmic fp64 work per walker-sample, in DFMA-equivalent
+# instructions (DADD, DMUL, DFMA each count 1; flops = 2 x this).
+K2_STENCIL = 18 * (ORDER + 1)          # 9 evaluation times x 2 polarisations x (p+1) taps
+K2_COEFF = 9 * (146)                   # 9 walker-dependent coefficient sets, 4.56 ops per tap
+K2_GEOM = 100                          # orbit, projections, delays
+K2_OPS = K2_STENCIL + K2_COEFF + K2_GEOM
+K2_BYTES = 16 + 48                     # h+,hx in, six links out
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=64, help=argparse.SUPPRESS)
+    ap.add_argument("--log2n", type=int, default=20, help=argparse.SUPPRESS)
+    ap.add_argument("--no-e2e", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--no-cpu-baseline", action="store_true", help=argparse.SUPPRESS)
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------- helpers
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU, sampled every 200 ms in the background."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax.append(float(parts[1]))
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)),
+                       power_w_max=float(max(power)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def shard_walkers(total_walkers: int, world: int, rank: int):
+    """Contiguous block of walkers owned by `rank` (the N>1 path: no data-path collective)."""
+    per = total_walkers // world
+    rem = total_walkers % world
+    lo = rank * per + min(rank, rem)
+    return lo, lo + per + (1 if rank < rem else 0)
+
+
+def dist_max(value: float, dist=None, device=None) -> float:
+    """max over ranks of a python float (identity without torch.distributed)."""
+    if dist is None or not dist.is_initialized():
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def oracle_sample_rate(inp, data, weight, kmin, kmax, window=1 << 14, cores=None):
+    """Time the fp64 CPU oracle, as it stands, on a bounded sample of the workload:
+    S1..S3 for `window` output samples of walker 0, then S4+S5 (three full-length FFTs + inner
+    product) for one walker.  Returns (evals_per_s, description, threads)."""
+    from oracle.binding import Oracle
+    orc = Oracle("d")
+    N = inp["N"]
+    n = lambda k: None if inp[k] is None else inp[k][:1].contiguous().cpu().numpy()
+    lo = N // 2
+    t0 = time.perf_counter()
+    orc.chain(inp["l"], inp["m"], n("amp"), n("phase"), n("iota"), n("phi"), n("psi"), n("lam"), n("beta_sky"),
+              inp["orbit"], inp["t0"], inp["dt"], inp["order"], inp["margin_y"], 20, 1, inp["margin_lo"],
+              inp["margin_hi"], alpha=n("alpha"), beta=n("beta"), gamma=n("gamma"), n_lo=lo, n_hi=lo + window,
+              want=("tdi",))
+    t_win = time.perf_counter() - t0
+    tdi = np.zeros((1, 3, N))
+    tdi[0, :, lo:lo + window] = 1e-22
+    t0 = time.perf_counter()
+    orc.loglike(tdi, data, weight, kmin, kmax)
+    t_fft = time.perf_counter() - t0
+    per_eval = t_win * (N / window) + t_fft
+    desc = (f"oracle (fp64 build, OpenMP) walker 0: S1-S3 on {window} of {N} output samples "
+            f"({t_win:.2f} s, scaled by N/{window}) + S4/S5 at full length ({t_fft:.2f} s)")
+    return 1.0 / per_eval, desc, orc.num_threads()
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2501_08261_b200 import synth
+    from oracle.binding import Oracle
+    N = 1 << args.log2n
+    inp = synth.make_inputs(CONFIG_ID, B=1, N=N)
+    kmin, kmax = synth.likelihood_band(N, inp["dt"])
+    orc = Oracle("d")
+    w = orc.psd_weights(N, inp["dt"], synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)
+    data = np.zeros((3, N // 2 + 1, 2))
+    vals, desc, threads = [], "", 1
+    for i in range(args.warmup + args.steps):
+        v, desc, threads = oracle_sample_rate(inp, data, w, kmin, kmax, window=1 << 12)
+        if i >= args.warmup:
+            vals.append(v)
+    value = float(len(vals) / sum(1.0 / v for v in vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value * 64,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": WORKLOAD, "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2501_08261_b200 import lib, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    lib.load()
+
+    B, N = args.batch, 1 << args.log2n
+    # weak scaling: every rank owns a full batch of B walkers (global batch = world * B);
+    # rank r uses seed offset r so the ranks hold different walkers of the same population
+    inp = synth.make_inputs(CONFIG_ID, device=device, B=B, N=N, seed=synth.SEED0 + CONFIG_ID + 1000 * rank)
+    dt, t0 = inp["dt"], inp["t0"]
+    kmin, kmax = synth.likelihood_band(N, dt)
+    w_host = lib.psd_weights(N, dt, synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)
+    weight = torch.from_numpy(w_host).to(device)
+    nf = N // 2 + 1
+    f64 = torch.float64
+    hp = torch.empty((B, N), dtype=f64, device=device)
+    hc = torch.empty_like(hp)
+    y = torch.empty((B, 6, N), dtype=f64, device=device)
+    tdi = torch.empty((B, 3, N), dtype=f64, device=device)
+    ll = torch.empty(B, dtype=f64, device=device)
+    dh = torch.empty(B, dtype=f64, device=device)
+    hh = torch.empty(B, dtype=f64, device=device)
+    plan = lib.Plan(B, N)
+    g = lambda k: inp[k]
+
+    def s1():
+        lib.modes_to_pol(B, N, inp["l"], inp["m"], g("amp"), g("phase"), g("alpha"), g("beta"), g("gamma"),
+                         g("iota"), g("phi"), g("psi"), None, hp, hc)
+
+    def s2():
+        lib.link_response(B, N, t0, dt, ORDER, inp["margin_y"], hp, hc, g("lam"), g("beta_sky"), inp["orbit"], y)
+
+    def s3():
+        lib.tdi2(B, N, t0, dt, ORDER, 20, 1, inp["margin_lo"], inp["margin_hi"], y, inp["orbit"], tdi)
+
+    # zero-noise injection: spectrum of walker 0
+    s1(); s2(); s3()
+    spec = torch.empty((B, 3, nf, 2), dtype=f64, device=device)
+    lib.spectrum(plan, B, N, tdi, spec)
+    data = spec[0].contiguous()
+    del spec
+    torch.cuda.synchronize()
+
+    def s45():
+        lib.loglike(plan, B, N, tdi, data, weight, kmin, kmax, ll, dh, hh)
+
+    # fp64 ALU peak, measured in this run (sustained ~1 s, all SMs): the roofline denominator
+    sink = torch.empty(148 * 8 * 256, dtype=f64, device=device)
+    lib.probe_dfma(20000, 148 * 8, 256, sink)
+    iters = 400000
+    ms = lib.probe_dfma(iters, 148 * 8, 256, sink)
+    dfma_peak_tflops = 2 * 8 * iters * 148 * 8 * 256 / (ms * 1e-3) / 1e12
+
+    stages = [("S1_modes_to_pol", s1), ("S2_link_response", s2), ("S3_tdi2", s3), ("S45_fft_loglike", s45)]
+    for _ in range(max(args.warmup, 3)):
+        for _, fn in stages:
+            fn()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(stages) + 1)] for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        ev[k][0].record()
+        for i, (_, fn) in enumerate(stages):
+            fn()
+            ev[k][i + 1].record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0][0].elapsed_time(ev[-1][-1])
+    total_ms = dist_max(total_ms, dist if world > 1 else None, device)
+    stage_ms = {nm: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)]))
+                for i, (nm, _) in enumerate(stages)}
+    ms_per_step = total_ms / args.steps
+    value = world * B / (ms_per_step * 1e-3)
+    loglike0 = float(ll[0].item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (S2, link response)
+    k2_ms = stage_ms["S2_link_response"]
+    ws = B * N
+    achieved = 2 * K2_OPS * ws / (k2_ms * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    roofline = {
+        "kernel": "k2_link_response<16>", "bound": "alu", "achieved": achieved, "peak": dfma_peak_tflops,
+        "unit": "TFLOP/s", "frac": achieved / dfma_peak_tflops, "traffic": None,
+        "peak_source": "DFMA probe measured in this run (lisa_td_probe_dfma, all SMs, ~1 s); nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2",
+        "ops_per_walker_sample": K2_OPS, "ms_per_launch": k2_ms,
+        "hbm_achieved_gbs": K2_BYTES * ws / (k2_ms * 1e-3) / 1e9,
+        "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
+        "hbm_frac": K2_BYTES * ws / (k2_ms * 1e-3) / 1e9 / hbm_peak,
+    }
+
+    # ---- end to end through the host API (pinned host buffers, copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        keys = ["amp", "phase", "alpha", "beta", "gamma", "iota", "phi", "psi", "lam", "beta_sky"]
+        host = {k: inp[k].cpu().pin_memory() for k in keys}
+        data_h, w_h = data.cpu().pin_memory(), weight.cpu().pin_memory()
+        out_h = torch.empty(B, dtype=f64).pin_memory()
+        # free the device-resident copies first: the pipeline owns its own chunk buffers
+        h2d = sum(host[k].numel() for k in keys) * 8 + (data_h.numel() + w_h.numel()) * 8
+        pipe = lib.Pipeline(16, N, len(inp["l"]), True)
+
+        def e2e_step():
+            lib.pipeline_host(pipe, B, N, inp["l"], inp["m"], host["amp"], host["phase"], host["alpha"],
+                              host["beta"], host["gamma"], host["iota"], host["phi"], host["psi"], host["lam"],
+                              host["beta_sky"], t0, dt, ORDER, inp["margin_y"], 20, inp["margin_lo"],
+                              inp["margin_hi"], inp["orbit"], data_h, w_h, kmin, kmax, out_h)
+        e2e_step()
+        torch.cuda.synchronize()
+        n_e2e = 3
+        t_start = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        t_e2e = (time.perf_counter() - t_start) / n_e2e
+        assert abs(float(out_h[0]) - loglike0) <= 1e-9 * abs(loglike0), (float(out_h[0]), loglike0)
+        e2e = {"value": B / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(B * 8),
+               "ms_per_step": t_e2e * 1e3, "api": "lisa_td_pipeline_host (chunks of 16 walkers, copy/compute streams)",
+               "steps": n_e2e}
+        pipe.close()
+
+    # ---- the oracle beside it (bounded sample, host cores)
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        inp1 = {k: (v[:1].cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
+        v, desc, threads = oracle_sample_rate(inp1, data.cpu().numpy(), w_host, kmin, kmax)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "global_batch": world * B, "N": N, "dt": dt, "order": ORDER,
+                   "l2": "inputs (6.8 GB per step) and every intermediate exceed the 126 MB L2",
+                   "parallelism": f"walker-split x{world}, no collective"},
+        "samples_per_s": value * N, "stage_ms": stage_ms, "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
+            "k1_modes_to_pol": 1, "k2_link_response": 1, "k3_tdi_merged": 1, "k5_inner_partial": 1,
+            "k5_inner_final": 1, "cufft (library)": "D2Z batch 192"},
+        "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
+    }
+    print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,181 @@
+/*
+ * lisa_td.h -- C ABI of liblisa_td.so: the per-likelihood hot path of the time-domain LISA
+ * pipeline of arXiv:2501.08261 on one NVIDIA B200 (sm_100a).
+ *
+ *   S1  modes -> h+, hx              Eq. 2.1-2.6   (psi at PAPER.md:306)
+ *   S2  h+, hx -> six link responses Eq. 2.7-2.8   (orbits PAPER.md:134)
+ *   S3  links -> TDI X,Y,Z -> A,E,T  Eq. 2.9-2.11  (interpolation PAPER.md:209)
+ *   S4  FFT of A,E,T (cuFFT)
+ *   S5  inner products -> log L      Eq. 2.12-2.13 (band PAPER.md:243)
+ *
+ * The readings taken where the paper is silent or garbled are listed in DESIGN.md section 2
+ * (A1..A18); the comments below name the ones each call depends on.
+ *
+ * General conventions
+ *  - Every array pointer is a DEVICE pointer unless its name ends in _host.  All arrays are
+ *    fp64, row-major, time fastest, and must be 16-byte aligned (LISA_TD_EALIGN otherwise).
+ *  - The caller owns every buffer.  The library allocates device memory only inside a
+ *    lisa_td_plan.  Inputs are never modified.
+ *  - Every call only ENQUEUES work on `stream` (a cudaStream_t passed as void*; NULL = the
+ *    legacy default stream) and returns without synchronising, except lisa_td_plan_create /
+ *    lisa_td_plan_destroy, lisa_td_pipeline_host and lisa_td_probe_dfma, which synchronise.
+ *  - Return value: LISA_TD_OK (0) or a negative lisa_td_status.  Argument errors are detected
+ *    on the host before any launch.  The library never throws, aborts or falls back to the
+ *    CPU.  lisa_td_last_error() returns a thread-local description of the last failure.
+ *  - Walkers b = 0..B-1, samples n = 0..N-1 at t_n = t0 + n*dt, `order` p odd in [1,63]
+ *    (p+1 Lagrange taps; p = 1 is the paper's linear interpolation).
+ *  - Link order everywhere: l = [1,2,3,-1,-2,-3] <-> (sender,receiver) =
+ *    [(3,2),(1,3),(2,1),(2,3),(3,1),(1,2)]  (y_{slr} notation of PAPER.md:132).
+ *
+ * Fractional-delay read (O-I of DESIGN.md): x(n - D) = sum_{j=-h+1..h} c_j(eps) x[n - K + j],
+ * K = ceil(D), eps = K - D, h = (p+1)/2, c_j(eps) = prod_{i != j} (eps - i)/(j - i), x = 0
+ * outside [0,N).
+ */
+#ifndef LISA_TD_H
+#define LISA_TD_H
+
+#if defined(__GNUC__)
+#define LISA_TD_API __attribute__((visibility("default")))
+#else
+#define LISA_TD_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LISA_TD_OK = 0,
+  LISA_TD_EINVAL = -1,   /* bad argument value (sizes, order, margins, NULL where not allowed) */
+  LISA_TD_EALIGN = -2,   /* a device pointer is not 16-byte aligned */
+  LISA_TD_ENOMEM = -3,   /* allocation failed / workspace too small */
+  LISA_TD_ECUDA = -4,    /* a CUDA or cuFFT call failed (see lisa_td_last_error) */
+  LISA_TD_ENOTIMPL = -5
+} lisa_td_status;
+
+LISA_TD_API const char* lisa_td_last_error(void);
+LISA_TD_API int lisa_td_version(void);
+
+/* Orbit description (host struct, copied at call time).
+ * kind 0 = STATIC : spacecraft positions r_static[spacecraft][xyz] in metres and the six light
+ *                   travel times L_static (seconds, link order) are constants.
+ * kind 1 = KEPLER1: reading A8 of DESIGN.md (analytic orbits, first-order solution of Kepler's
+ *                   equation, breathing unequal arms; L_l(t) = |r_r(t) - r_s(t)|/c). */
+typedef struct {
+  int kind;
+  double L_m, a_m, year_s, phase0, t_ref;
+  double r_static[3][3];
+  double L_static[6];
+} lisa_td_orbit;
+
+/* S1 -- Eq. 2.4-2.6 (single-sum form; readings A1-A6).
+ *   h+ - i hx = e^{2 i psi} sum_k [ h_k frakD^l_{m,2}(R) + (-1)^l conj(h_k) frakD^l_{-m,2}(R) ] sqrt((2l+1)/4pi)
+ *   h_k = amp_k e^{-i phase_k},  R = R(alpha,beta,gamma)(t) . R(euler0) . R(phi, iota, 0)
+ * l_host/m_host: n_modes (<= 16) mode labels, 2 <= l <= 8, 0 <= m <= l (the -m partner is implied).
+ * amp, phase: [B][n_modes][N].  alpha,beta,gamma: [B][N] each, or all three NULL (aligned spin).
+ * iota, phi, psi: [B].  euler0: [B][3] constant J->L0 angles or NULL.  hplus, hcross: [B][N]. */
+LISA_TD_API int lisa_td_modes_to_pol(int B, long long N, int n_modes, const int* l_host, const int* m_host,
+                         const double* amp, const double* phase, const double* alpha,
+                         const double* beta, const double* gamma, const double* iota,
+                         const double* phi, const double* psi, const double* euler0,
+                         double* hplus, double* hcross, void* stream);
+
+/* S2 -- Eq. 2.7-2.8 (readings A7, A8, A11).  For every link (s,l,r) and sample n, with r_i, L_l
+ * at the reception time t_n:
+ *   y = [ x+ (h+(n-Ds) - h+(n-Dr)) + 2 xx (hx(n-Ds) - hx(n-Dr)) ] / ( 2 (1 - k.n) ),
+ *   Ds = (L_l + k.r_s/c)/dt, Dr = (k.r_r/c)/dt, fractional-delay reads of order p.
+ * hplus, hcross: [B][N] on the output grid.  lambda, beta_sky: [B] ecliptic longitude/latitude.
+ * y: [B][6][N]; samples outside [margin_y, N - margin_y) are written as exact zeros.
+ * margin_y must cover the stencil reach: margin_y >= ceil(max|D|) + (p+1)/2 for the given orbit
+ * (LISA_TD_EINVAL otherwise; the bound used is max_i |r_i|/c + max_l L_l). */
+LISA_TD_API int lisa_td_link_response(int B, long long N, double t0, double dt, int order, long long margin_y,
+                          const double* hplus, const double* hcross, const double* lambda,
+                          const double* beta_sky, const lisa_td_orbit* orbit_host, double* y,
+                          void* stream);
+
+/* A12 -- link-level common laser noise y_l[n] = p(n - L_l(t_n)/dt) - p[n] (zero outside
+ * [margin, N - margin)); p: [N], y: [6][N].  Used to check TDI laser-noise suppression. */
+LISA_TD_API int lisa_td_laser_links(long long N, double t0, double dt, int order, long long margin,
+                        const double* p, const lisa_td_orbit* orbit_host, double* y, void* stream);
+
+/* S3 -- Eq. 2.9 (generation 15) / Eq. 2.10 with the y123 block corrected (generation 20, reading
+ * A9), Y and Z by cyclic permutation, optionally A,E,T of Eq. 2.11.  Every delayed read is a
+ * fractional-delay read of one y series at D = (sum of the listed L_l(t_n))/dt (A10: summed, all
+ * L at the output time).  y: [B][6][N].  tdi: [B][3][N], out_kind 0 = X,Y,Z, 1 = A,E,T; samples
+ * outside [margin_lo, N - margin_hi) are exact zeros.  Requires margin_lo >= ceil(7 Lmax/dt) +
+ * (p+1)/2 (3 Lmax for generation 15) and margin_hi >= (p+1)/2. */
+LISA_TD_API int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+                 long long margin_lo, long long margin_hi, const double* y,
+                 const lisa_td_orbit* orbit_host, double* tdi, void* stream);
+
+/* S2+S3 in one call: h+,hx -> tdi.  The six links of a walker chunk live in `workspace`
+ * (device, >= lisa_td_response_tdi_workspace_bytes(B,N) bytes), never in a caller array. */
+LISA_TD_API long long lisa_td_response_tdi_workspace_bytes(int B, long long N);
+LISA_TD_API int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, long long margin_y,
+                         int generation, int out_kind, long long margin_lo, long long margin_hi,
+                         const double* hplus, const double* hcross, const double* lambda,
+                         const double* beta_sky, const lisa_td_orbit* orbit_host, double* tdi,
+                         void* workspace, long long workspace_bytes, void* stream);
+
+/* S4+S5 plan: owns the cuFFT plan (batched real-to-complex, length N), the spectrum scratch
+ * and the partial-sum scratch for up to B walkers. */
+typedef struct lisa_td_plan lisa_td_plan;
+LISA_TD_API int lisa_td_plan_create(lisa_td_plan** out, int B, long long N);
+LISA_TD_API int lisa_td_plan_destroy(lisa_td_plan* plan);
+
+/* S4+S5 -- Eq. 2.12-2.13 (readings A13, A17):  H_c[k] = sum_n tdi_c[n] e^{-2 pi i k n/N},
+ *   (d|h)_b = sum_c sum_{k=kmin..kmax} w_c[k] Re( D_c[k] conj(H_{b,c}[k]) ),
+ *   (h|h)_b = sum_c sum_k w_c[k] |H_{b,c}[k]|^2,   log L_b = (d|h)_b - (h|h)_b / 2.
+ * tdi: [B][3][N] (A,E,T); data_spec: [3][N/2+1][2] (re,im); weight: [3][N/2+1] =
+ * 4 df dt^2 / S_c(f_k); 0 <= kmin <= kmax <= N/2.  loglike: [B]; dh, hh: [B] or NULL. */
+LISA_TD_API int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const double* tdi,
+                    const double* data_spec, const double* weight, long long kmin, long long kmax,
+                    double* loglike, double* dh, double* hh, void* stream);
+
+/* Spectrum only (used to build the zero-noise injection): tdi [B][3][N] ->
+ * spec [B][3][N/2+1][2]. */
+LISA_TD_API int lisa_td_spectrum(lisa_td_plan* plan, int B, long long N, const double* tdi, double* spec,
+                     void* stream);
+
+/* Host helper, outside the timed path: Eq. 2.14-2.15 with readings A14, A15, A17.
+ * weight_host: [3][N/2+1] (A,E,T) = 4 df dt^2 / S_c(k df), 0 at k = 0; generation 20 multiplies
+ * the PSDs by 4 sin^2(4 pi f arm_s). */
+LISA_TD_API int lisa_td_psd_weights(long long N, double dt, double acc_noise, double oms_noise, double arm_s,
+                        int generation, double* weight_host);
+
+/* Whole path S1..S5 from HOST buffers (the end-to-end call).  All *_host arrays are host memory
+ * (pinned for full copy bandwidth); layouts as in the calls above.  Walkers are processed in
+ * chunks of the plan's capacity; host->device copies of chunk i+1 overlap the kernels of chunk
+ * i on two internal streams.  Synchronises before returning.  alpha/beta/gamma_host may all be
+ * NULL.  loglike_host: [B]; dh_host, hh_host: [B] or NULL. */
+typedef struct lisa_td_pipeline lisa_td_pipeline;
+LISA_TD_API int lisa_td_pipeline_create(lisa_td_pipeline** out, int chunk_B, long long N, int n_modes,
+                            int twisted);
+LISA_TD_API int lisa_td_pipeline_destroy(lisa_td_pipeline* p);
+LISA_TD_API int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                          const int* m_host, const double* amp_host, const double* phase_host,
+                          const double* alpha_host, const double* beta_host,
+                          const double* gamma_host, const double* iota_host,
+                          const double* phi_host, const double* psi_host,
+                          const double* lambda_host, const double* beta_sky_host, double t0,
+                          double dt, int order, long long margin_y, int generation,
+                          long long margin_lo, long long margin_hi,
+                          const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                          const double* weight_host, long long kmin, long long kmax,
+                          double* loglike_host, double* dh_host, double* hh_host);
+
+/* Measurement support: a register-resident chain of `iters` x 8 dependent-free DFMA per thread on
+ * `blocks` x `threads`; returns the elapsed milliseconds (CUDA events) in *ms_host and writes one
+ * double per thread to sink (device, blocks*threads doubles) so the work is not optimised away.
+ * FLOP count = 2 * 8 * iters * blocks * threads. */
+LISA_TD_API int lisa_td_probe_dfma(long long iters, int blocks, int threads, double* sink, float* ms_host,
+                       void* stream);
+
+/* Testing switch: non-zero routes S2/S3 through the generic (runtime-order, unmerged) kernels
+ * even where a specialised instantiation exists, so the tests can cover both. */
+LISA_TD_API void lisa_td_debug_force_generic(int on);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LISA_TD_H */

@@ -1,0 +1,556 @@
+// api.cu -- the extern "C" boundary of liblisa_td (include/lisa_td.h): argument validation,
+// host-side preparation of the constant tables handed to the kernels, the end-to-end host
+// pipeline and the DFMA probe.  No arithmetic of the method runs on the host; there is no
+// CPU fallback.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "common.cuh"
+
+namespace lisa {
+
+// ------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+
+int set_error(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+int check_cuda(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return LISA_TD_OK;
+  return set_error(e == cudaErrorMemoryAllocation ? LISA_TD_ENOMEM : LISA_TD_ECUDA, "%s: %s (%s)", what,
+                   cudaGetErrorString(e), cudaGetErrorName(e));
+}
+
+// ------------------------------------------------------------------ constant tables
+void make_lagw(int order, LagW* out) {
+  const int H = (order + 1) / 2;
+  for (int i = 0; i < MAX_HALF; ++i) out->w[i] = 0.0;
+  for (int k = 1; k <= H; ++k) {
+    long double f = 1.0L;  // (k+H-1)! (H-k)!
+    for (int i = 2; i <= k + H - 1; ++i) f *= i;
+    for (int i = 2; i <= H - k; ++i) f *= i;
+    long double w = 1.0L / f;
+    if ((H - k) & 1) w = -w;
+    out->w[k - 1] = (double)w;
+  }
+}
+
+// KEPLER1 on the host (long double), used only to bound |r| and L for margin validation.
+static void kepler1_host(const lisa_td_orbit* o, long double t, long double r[3][3]) {
+  const long double PI_L = 3.14159265358979323846264338327950288L;
+  long double a = o->a_m, delta = (long double)o->L_m / (2 * a), sq3 = sqrtl(3.0L);
+  long double e = sqrtl(1 + 2 * delta / sq3 + 4 * delta * delta / 3) - 1;
+  long double inc = atanl(delta / (1 + delta / sq3));
+  for (int k = 0; k < 3; ++k) {
+    long double sigma = 2 * PI_L * k / 3;
+    long double M = 2 * PI_L * (t - o->t_ref) / o->year_s - sigma - o->phase0;
+    long double psi = M + e * sinl(M);
+    long double x = a * (cosl(psi) - e) * cosl(inc), y = a * sqrtl(1 - e * e) * sinl(psi);
+    long double z = a * (cosl(psi) - e) * sinl(inc);
+    r[k][0] = cosl(sigma) * x - sinl(sigma) * y;
+    r[k][1] = sinl(sigma) * x + cosl(sigma) * y;
+    r[k][2] = z;
+  }
+}
+
+int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
+  if (!o) return set_error(LISA_TD_EINVAL, "orbit_host is NULL");
+  memset(d, 0, sizeof(*d));
+  d->kind = o->kind;
+  if (o->kind == 0) {
+    double mr = 0.0, mL = 0.0;
+    for (int k = 0; k < 3; ++k) {
+      double s = 0.0;
+      for (int j = 0; j < 3; ++j) {
+        d->r[k][j] = o->r_static[k][j];
+        s += o->r_static[k][j] * o->r_static[k][j];
+      }
+      mr = fmax(mr, sqrt(s));
+    }
+    for (int l = 0; l < 6; ++l) {
+      if (!(o->L_static[l] >= 0.0)) return set_error(LISA_TD_EINVAL, "orbit: L_static[%d] must be >= 0", l);
+      d->L[l] = o->L_static[l];
+      mL = fmax(mL, o->L_static[l]);
+    }
+    d->max_r_over_c = mr / C_LIGHT;
+    d->max_L = mL;
+    return LISA_TD_OK;
+  }
+  if (o->kind != 1) return set_error(LISA_TD_EINVAL, "orbit: unknown kind %d", o->kind);
+  if (!(o->a_m > 0) || !(o->L_m > 0) || !(o->year_s > 0))
+    return set_error(LISA_TD_EINVAL, "orbit: KEPLER1 needs a_m, L_m, year_s > 0");
+  const long double PI_L = 3.14159265358979323846264338327950288L;
+  long double a = o->a_m, delta = (long double)o->L_m / (2 * a), sq3 = sqrtl(3.0L);
+  long double e = sqrtl(1 + 2 * delta / sq3 + 4 * delta * delta / 3) - 1;
+  long double inc = atanl(delta / (1 + delta / sq3));
+  long double bq = sqrtl(1 - e * e);
+  d->w = (double)(2 * PI_L / o->year_s);
+  d->t_ref = o->t_ref;
+  d->phase0 = o->phase0;
+  d->a = o->a_m;
+  d->a_over_c = (double)(a / (long double)C_LIGHT);
+  d->e = (double)e;
+  d->ci = (double)cosl(inc);
+  d->si = (double)sinl(inc);
+  d->dci = (double)(-2 * sinl(inc / 2) * sinl(inc / 2));
+  d->bq = (double)bq;
+  d->dbq = (double)(-e * e / (1 + bq));
+  for (int k = 0; k < 3; ++k) {
+    d->cs[k] = (double)cosl(2 * PI_L * k / 3);
+    d->sn[k] = (double)sinl(2 * PI_L * k / 3);
+  }
+  // bounds over one orbital period (the motion is periodic), 4096 points, 0.1 % head-room
+  long double mr = 0, mL = 0;
+  for (int i = 0; i < 4096; ++i) {
+    long double r[3][3];
+    kepler1_host(o, o->t_ref + (long double)o->year_s * i / 4096, r);
+    for (int k = 0; k < 3; ++k) {
+      mr = fmaxl(mr, sqrtl(r[k][0] * r[k][0] + r[k][1] * r[k][1] + r[k][2] * r[k][2]));
+      const int k2 = (k + 1) % 3;
+      long double dx = r[k][0] - r[k2][0], dy = r[k][1] - r[k2][1], dz = r[k][2] - r[k2][2];
+      mL = fmaxl(mL, sqrtl(dx * dx + dy * dy + dz * dz));
+    }
+  }
+  d->max_r_over_c = (double)(mr * 1.001L / C_LIGHT);
+  d->max_L = (double)(mL * 1.001L / C_LIGHT);
+  return LISA_TD_OK;
+}
+
+// kernels (other translation units)
+int run_modes_to_pol(int, long long, int, const int*, const int*, const double*, const double*,
+                     const double*, const double*, const double*, const double*, const double*,
+                     const double*, const double*, double*, double*, cudaStream_t);
+int run_link_response(int, long long, double, double, int, long long, const double*, const double*,
+                      const double*, const double*, const OrbitDev&, double*, cudaStream_t);
+int run_laser_links(long long, double, double, int, long long, const double*, const OrbitDev&,
+                    double*, cudaStream_t);
+int run_tdi(int, long long, double, double, int, int, int, long long, long long, const double*,
+            const OrbitDev&, double*, cudaStream_t);
+struct Plan;
+int plan_create(Plan**, int, long long);
+int plan_destroy(Plan*);
+int run_spectrum(Plan*, int, long long, const double*, double*, cudaStream_t);
+int run_loglike(Plan*, int, long long, const double*, const double*, const double*, long long,
+                long long, double*, double*, double*, cudaStream_t);
+extern int g_force_generic;
+
+// ------------------------------------------------------------------ validation helpers
+static int check_common(const char* fn, int B, long long N, double dt, int order) {
+  if (B <= 0) return set_error(LISA_TD_EINVAL, "%s: B must be > 0 (got %d)", fn, B);
+  if (N <= 0) return set_error(LISA_TD_EINVAL, "%s: N must be > 0 (got %lld)", fn, N);
+  if (!(dt > 0)) return set_error(LISA_TD_EINVAL, "%s: dt must be > 0", fn);
+  if (order < 1 || order > 63 || !(order & 1))
+    return set_error(LISA_TD_EINVAL, "%s: order must be odd in [1,63] (got %d)", fn, order);
+  if (B > 65535) return set_error(LISA_TD_EINVAL, "%s: B must be <= 65535", fn);
+  return LISA_TD_OK;
+}
+#define REQUIRE_PTR(fn, p)                                                              \
+  do {                                                                                  \
+    if (!(p)) return set_error(LISA_TD_EINVAL, "%s: %s is NULL", fn, #p);               \
+    if (!aligned16(p)) return set_error(LISA_TD_EALIGN, "%s: %s is not 16-byte aligned", fn, #p); \
+  } while (0)
+#define OPTIONAL_PTR(fn, p)                                                             \
+  do {                                                                                  \
+    if ((p) && !aligned16(p)) return set_error(LISA_TD_EALIGN, "%s: %s is not 16-byte aligned", fn, #p); \
+  } while (0)
+
+static int check_margin_y(const char* fn, long long N, double dt, int order, long long margin_y, const OrbitDev& od) {
+  const long long need = (long long)ceil((od.max_r_over_c + od.max_L) / dt) + (order + 1) / 2;
+  if (margin_y < need)
+    return set_error(LISA_TD_EINVAL, "%s: margin_y=%lld does not cover the stencil reach %lld", fn, margin_y, need);
+  if (margin_y > 8192) return set_error(LISA_TD_EINVAL, "%s: margin_y=%lld too large (max 8192)", fn, margin_y);
+  if (N < 2 * margin_y) return set_error(LISA_TD_EINVAL, "%s: N=%lld must be >= 2*margin_y", fn, N);
+  return LISA_TD_OK;
+}
+static int check_margin_tdi(const char* fn, long long N, double dt, int order, int generation,
+                            long long margin_lo, long long margin_hi, const OrbitDev& od) {
+  if (generation != 15 && generation != 20)
+    return set_error(LISA_TD_EINVAL, "%s: generation must be 15 or 20 (got %d)", fn, generation);
+  const int h = (order + 1) / 2;
+  const long long need_lo = (long long)ceil((generation == 20 ? 7 : 3) * od.max_L / dt) + h;
+  if (margin_lo < need_lo)
+    return set_error(LISA_TD_EINVAL, "%s: margin_lo=%lld does not cover the stencil reach %lld", fn, margin_lo, need_lo);
+  if (margin_hi < h)
+    return set_error(LISA_TD_EINVAL, "%s: margin_hi=%lld must be >= (order+1)/2 = %d", fn, margin_hi, h);
+  if (N < margin_lo + margin_hi) return set_error(LISA_TD_EINVAL, "%s: N=%lld smaller than the margins", fn, N);
+  return LISA_TD_OK;
+}
+
+}  // namespace lisa
+
+using namespace lisa;
+
+// ====================================================================== C ABI
+extern "C" {
+
+const char* lisa_td_last_error(void) { return g_err; }
+int lisa_td_version(void) { return 100; }
+void lisa_td_debug_force_generic(int on) { g_force_generic = on; }
+
+int lisa_td_modes_to_pol(int B, long long N, int n_modes, const int* l_host, const int* m_host,
+                         const double* amp, const double* phase, const double* alpha,
+                         const double* beta, const double* gamma, const double* iota,
+                         const double* phi, const double* psi, const double* euler0,
+                         double* hplus, double* hcross, void* stream) {
+  const char* fn = "lisa_td_modes_to_pol";
+  if (B <= 0 || B > 65535) return set_error(LISA_TD_EINVAL, "%s: B must be in [1,65535] (got %d)", fn, B);
+  if (N <= 0) return set_error(LISA_TD_EINVAL, "%s: N must be > 0", fn);
+  if (n_modes <= 0 || n_modes > 16) return set_error(LISA_TD_EINVAL, "%s: n_modes must be in [1,16]", fn);
+  if (!l_host || !m_host) return set_error(LISA_TD_EINVAL, "%s: l_host / m_host is NULL", fn);
+  for (int k = 0; k < n_modes; ++k)
+    if (l_host[k] < 2 || l_host[k] > 8 || m_host[k] < -l_host[k] || m_host[k] > l_host[k])
+      return set_error(LISA_TD_EINVAL, "%s: mode %d = (%d,%d) outside 2<=l<=8, |m|<=l", fn, k, l_host[k], m_host[k]);
+  REQUIRE_PTR(fn, amp); REQUIRE_PTR(fn, phase); REQUIRE_PTR(fn, iota); REQUIRE_PTR(fn, phi);
+  REQUIRE_PTR(fn, psi); REQUIRE_PTR(fn, hplus); REQUIRE_PTR(fn, hcross);
+  const int nang = (alpha != 0) + (beta != 0) + (gamma != 0);
+  if (nang != 0 && nang != 3) return set_error(LISA_TD_EINVAL, "%s: alpha, beta, gamma must be all NULL or all given", fn);
+  OPTIONAL_PTR(fn, alpha); OPTIONAL_PTR(fn, beta); OPTIONAL_PTR(fn, gamma); OPTIONAL_PTR(fn, euler0);
+  return run_modes_to_pol(B, N, n_modes, l_host, m_host, amp, phase, alpha, beta, gamma, iota, phi, psi,
+                          euler0, hplus, hcross, (cudaStream_t)stream);
+}
+
+int lisa_td_link_response(int B, long long N, double t0, double dt, int order, long long margin_y,
+                          const double* hplus, const double* hcross, const double* lambda,
+                          const double* beta_sky, const lisa_td_orbit* orbit_host, double* y,
+                          void* stream) {
+  const char* fn = "lisa_td_link_response";
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  REQUIRE_PTR(fn, hplus); REQUIRE_PTR(fn, hcross); REQUIRE_PTR(fn, lambda); REQUIRE_PTR(fn, beta_sky);
+  REQUIRE_PTR(fn, y);
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
+  return run_link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lambda, beta_sky, od, y,
+                           (cudaStream_t)stream);
+}
+
+int lisa_td_laser_links(long long N, double t0, double dt, int order, long long margin,
+                        const double* p, const lisa_td_orbit* orbit_host, double* y, void* stream) {
+  const char* fn = "lisa_td_laser_links";
+  int rc = check_common(fn, 1, N, dt, order);
+  if (rc) return rc;
+  REQUIRE_PTR(fn, p); REQUIRE_PTR(fn, y);
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  const long long need = (long long)ceil(od.max_L / dt) + (order + 1) / 2;
+  if (margin < need || N < 2 * margin)
+    return set_error(LISA_TD_EINVAL, "%s: margin=%lld must be >= %lld and N >= 2*margin", fn, margin, need);
+  return run_laser_links(N, t0, dt, order, margin, p, od, y, (cudaStream_t)stream);
+}
+
+int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+                 long long margin_lo, long long margin_hi, const double* y,
+                 const lisa_td_orbit* orbit_host, double* tdi, void* stream) {
+  const char* fn = "lisa_td_tdi2";
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (out_kind != 0 && out_kind != 1) return set_error(LISA_TD_EINVAL, "%s: out_kind must be 0 (XYZ) or 1 (AET)", fn);
+  REQUIRE_PTR(fn, y); REQUIRE_PTR(fn, tdi);
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+  return run_tdi(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi,
+                 (cudaStream_t)stream);
+}
+
+long long lisa_td_response_tdi_workspace_bytes(int B, long long N) {
+  if (B <= 0 || N <= 0) return 0;
+  return (long long)sizeof(double) * 6 * (long long)B * N;
+}
+
+int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, long long margin_y,
+                         int generation, int out_kind, long long margin_lo, long long margin_hi,
+                         const double* hplus, const double* hcross, const double* lambda,
+                         const double* beta_sky, const lisa_td_orbit* orbit_host, double* tdi,
+                         void* workspace, long long workspace_bytes, void* stream) {
+  const char* fn = "lisa_td_response_tdi";
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (out_kind != 0 && out_kind != 1) return set_error(LISA_TD_EINVAL, "%s: out_kind must be 0 or 1", fn);
+  REQUIRE_PTR(fn, hplus); REQUIRE_PTR(fn, hcross); REQUIRE_PTR(fn, lambda); REQUIRE_PTR(fn, beta_sky);
+  REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, workspace);
+  if (workspace_bytes < lisa_td_response_tdi_workspace_bytes(B, N))
+    return set_error(LISA_TD_ENOMEM, "%s: workspace of %lld bytes is smaller than the %lld needed", fn,
+                     workspace_bytes, lisa_td_response_tdi_workspace_bytes(B, N));
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+  double* y = static_cast<double*>(workspace);
+  if ((rc = run_link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lambda, beta_sky, od, y,
+                              (cudaStream_t)stream)))
+    return rc;
+  return run_tdi(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi,
+                 (cudaStream_t)stream);
+}
+
+struct lisa_td_plan {
+  lisa::Plan* p;
+};
+
+int lisa_td_plan_create(lisa_td_plan** out, int B, long long N) {
+  const char* fn = "lisa_td_plan_create";
+  if (!out) return set_error(LISA_TD_EINVAL, "%s: out is NULL", fn);
+  if (B <= 0 || B > 65535 || N < 2 || (N & 1))
+    return set_error(LISA_TD_EINVAL, "%s: need 0 < B <= 65535 and even N >= 2", fn);
+  lisa::Plan* p = nullptr;
+  int rc = plan_create(&p, B, N);
+  if (rc) return rc;
+  *out = new lisa_td_plan{p};
+  return LISA_TD_OK;
+}
+int lisa_td_plan_destroy(lisa_td_plan* plan) {
+  if (!plan) return LISA_TD_OK;
+  plan_destroy(plan->p);
+  delete plan;
+  return LISA_TD_OK;
+}
+
+static int check_band(const char* fn, long long N, long long kmin, long long kmax) {
+  if (kmin < 0 || kmin > kmax || kmax > N / 2)
+    return set_error(LISA_TD_EINVAL, "%s: need 0 <= kmin <= kmax <= N/2 (got %lld, %lld)", fn, kmin, kmax);
+  return LISA_TD_OK;
+}
+
+int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const double* tdi,
+                    const double* data_spec, const double* weight, long long kmin, long long kmax,
+                    double* loglike, double* dh, double* hh, void* stream) {
+  const char* fn = "lisa_td_loglike";
+  if (!plan) return set_error(LISA_TD_EINVAL, "%s: plan is NULL", fn);
+  if (B <= 0) return set_error(LISA_TD_EINVAL, "%s: B must be > 0", fn);
+  int rc = check_band(fn, N, kmin, kmax);
+  if (rc) return rc;
+  REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, data_spec); REQUIRE_PTR(fn, weight); REQUIRE_PTR(fn, loglike);
+  return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream);
+}
+
+int lisa_td_spectrum(lisa_td_plan* plan, int B, long long N, const double* tdi, double* spec, void* stream) {
+  const char* fn = "lisa_td_spectrum";
+  if (!plan) return set_error(LISA_TD_EINVAL, "%s: plan is NULL", fn);
+  if (B <= 0) return set_error(LISA_TD_EINVAL, "%s: B must be > 0", fn);
+  REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, spec);
+  return run_spectrum(plan->p, B, N, tdi, spec, (cudaStream_t)stream);
+}
+
+int lisa_td_psd_weights(long long N, double dt, double acc_noise, double oms_noise, double arm_s,
+                        int generation, double* weight_host) {
+  const char* fn = "lisa_td_psd_weights";
+  if (N < 2 || !(dt > 0) || !weight_host) return set_error(LISA_TD_EINVAL, "%s: bad arguments", fn);
+  if (generation != 15 && generation != 20) return set_error(LISA_TD_EINVAL, "%s: generation must be 15 or 20", fn);
+  const long long nf = N / 2 + 1;
+  const double PI = 3.14159265358979323846;
+  const double df = 1.0 / ((double)N * dt);
+  for (int c = 0; c < 3; ++c) weight_host[(size_t)c * nf] = 0.0;
+  for (long long k = 1; k < nf; ++k) {
+    const double f = k * df, om = 2 * PI * f, oc = om / C_LIGHT;
+    // Eq. 2.14 (shapes as printed; amplitudes are arguments, A15)
+    const double r1 = 4e-4 / f, r2 = f / 0.008, r3 = 0.002 / f;
+    const double s_acc = acc_noise * acc_noise * (1 + r1 * r1) * (1 + r2 * r2 * r2 * r2) / (om * om * om * om) * oc * oc;
+    const double s_op = oms_noise * oms_noise * (1 + r3 * r3 * r3 * r3) * oc * oc;
+    // Eq. 2.15 with x = 2 pi f L/c (A14)
+    const double x = om * arm_s, sx = sin(x), cx = cos(x), sh = sin(0.5 * x);
+    double s_ae = 8 * sx * sx * (2 * s_acc * (3 + 2 * cx + cos(2 * x)) + s_op * (2 + cx));
+    double s_t = 16 * s_op * (1 - cx) * sx * sx + 128 * s_acc * sx * sx * sh * sh * sh * sh;
+    if (generation == 20) {
+      const double g = 4 * sin(2 * x) * sin(2 * x);
+      s_ae *= g;
+      s_t *= g;
+    }
+    const double num = 4 * df * dt * dt;
+    weight_host[k] = num / s_ae;
+    weight_host[nf + k] = num / s_ae;
+    weight_host[2 * nf + k] = num / s_t;
+  }
+  return LISA_TD_OK;
+}
+
+// ---------------------------------------------------------------------- host pipeline
+struct lisa_td_pipeline {
+  int chunk_B, n_modes, twisted;
+  long long N, nf;
+  cudaStream_t s_copy, s_comp;
+  cudaEvent_t copied[2], done[2];
+  double* in[2];      // per buffer: amp, phase [cB][M][N], (alpha,beta,gamma [cB][N]), 5 scalars [cB]
+  double *hp, *hc, *y, *tdi, *ll;  // ll: [3][cB] (loglike, dh, hh)
+  double *data_spec, *weight;
+  lisa::Plan* plan;
+  size_t in_doubles;
+};
+
+int lisa_td_pipeline_destroy(lisa_td_pipeline* p) {
+  if (!p) return LISA_TD_OK;
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(p->in[i]);
+    if (p->copied[i]) cudaEventDestroy(p->copied[i]);
+    if (p->done[i]) cudaEventDestroy(p->done[i]);
+  }
+  cudaFree(p->hp); cudaFree(p->hc); cudaFree(p->y); cudaFree(p->tdi); cudaFree(p->ll);
+  cudaFree(p->data_spec); cudaFree(p->weight);
+  if (p->plan) plan_destroy(p->plan);
+  if (p->s_copy) cudaStreamDestroy(p->s_copy);
+  if (p->s_comp) cudaStreamDestroy(p->s_comp);
+  delete p;
+  return LISA_TD_OK;
+}
+
+int lisa_td_pipeline_create(lisa_td_pipeline** out, int chunk_B, long long N, int n_modes, int twisted) {
+  const char* fn = "lisa_td_pipeline_create";
+  if (!out || chunk_B <= 0 || N < 2 || (N & 1) || n_modes <= 0 || n_modes > 16)
+    return set_error(LISA_TD_EINVAL, "%s: bad arguments", fn);
+  lisa_td_pipeline* p = new lisa_td_pipeline();
+  memset(p, 0, sizeof(*p));
+  p->chunk_B = chunk_B; p->N = N; p->nf = N / 2 + 1; p->n_modes = n_modes; p->twisted = twisted;
+  const size_t cB = chunk_B;
+  p->in_doubles = cB * (2 * (size_t)n_modes + (twisted ? 3 : 0)) * N + 8 * cB + 16;
+  int rc = LISA_TD_OK;
+#define PIPE_TRY(call) do { if (rc == LISA_TD_OK) rc = check_cuda((call), #call); } while (0)
+  PIPE_TRY(cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking));
+  PIPE_TRY(cudaStreamCreateWithFlags(&p->s_comp, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) {
+    PIPE_TRY(cudaMalloc(&p->in[i], sizeof(double) * p->in_doubles));
+    PIPE_TRY(cudaEventCreateWithFlags(&p->copied[i], cudaEventDisableTiming));
+    PIPE_TRY(cudaEventCreateWithFlags(&p->done[i], cudaEventDisableTiming));
+  }
+  PIPE_TRY(cudaMalloc(&p->hp, sizeof(double) * cB * N));
+  PIPE_TRY(cudaMalloc(&p->hc, sizeof(double) * cB * N));
+  PIPE_TRY(cudaMalloc(&p->y, sizeof(double) * cB * 6 * N));
+  PIPE_TRY(cudaMalloc(&p->tdi, sizeof(double) * cB * 3 * N));
+  PIPE_TRY(cudaMalloc(&p->ll, sizeof(double) * (4 * cB + 8)));
+  PIPE_TRY(cudaMalloc(&p->data_spec, sizeof(double) * 6 * p->nf));
+  PIPE_TRY(cudaMalloc(&p->weight, sizeof(double) * 4 * p->nf));
+#undef PIPE_TRY
+  if (rc == LISA_TD_OK) rc = plan_create(&p->plan, chunk_B, N);
+  if (rc != LISA_TD_OK) {
+    lisa_td_pipeline_destroy(p);
+    return rc;
+  }
+  *out = p;
+  return LISA_TD_OK;
+}
+
+int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                          const int* m_host, const double* amp_host, const double* phase_host,
+                          const double* alpha_host, const double* beta_host,
+                          const double* gamma_host, const double* iota_host,
+                          const double* phi_host, const double* psi_host,
+                          const double* lambda_host, const double* beta_sky_host, double t0,
+                          double dt, int order, long long margin_y, int generation,
+                          long long margin_lo, long long margin_hi,
+                          const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                          const double* weight_host, long long kmin, long long kmax,
+                          double* loglike_host, double* dh_host, double* hh_host) {
+  const char* fn = "lisa_td_pipeline_host";
+  if (!p) return set_error(LISA_TD_EINVAL, "%s: pipeline is NULL", fn);
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (N != p->N || n_modes != p->n_modes) return set_error(LISA_TD_EINVAL, "%s: N / n_modes differ from the pipeline's", fn);
+  const bool tw = alpha_host != nullptr;
+  if (tw != (p->twisted != 0)) return set_error(LISA_TD_EINVAL, "%s: twisted flag differs from the pipeline's", fn);
+  if (!amp_host || !phase_host || !iota_host || !phi_host || !psi_host || !lambda_host || !beta_sky_host ||
+      !data_spec_host || !weight_host || !loglike_host || !l_host || !m_host || (tw && (!beta_host || !gamma_host)))
+    return set_error(LISA_TD_EINVAL, "%s: a required host pointer is NULL", fn);
+  for (int k = 0; k < n_modes; ++k)
+    if (l_host[k] < 2 || l_host[k] > 8 || m_host[k] < -l_host[k] || m_host[k] > l_host[k])
+      return set_error(LISA_TD_EINVAL, "%s: mode %d outside 2<=l<=8, |m|<=l", fn, k);
+  if ((rc = check_band(fn, N, kmin, kmax))) return rc;
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+
+  const size_t M = n_modes, cB = p->chunk_B;
+  LISA_CUDA(cudaMemcpyAsync(p->data_spec, data_spec_host, sizeof(double) * 6 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
+  LISA_CUDA(cudaMemcpyAsync(p->weight, weight_host, sizeof(double) * 3 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
+  int it = 0;
+  for (int b0 = 0; b0 < B; b0 += (int)cB, ++it) {
+    const int buf = it & 1;
+    const size_t nb = (size_t)((B - b0) < (int)cB ? (B - b0) : (int)cB);
+    double* d = p->in[buf];
+    double* d_amp = d;
+    double* d_pha = d_amp + cB * M * N;
+    double* d_al = d_pha + cB * M * N;
+    double* d_be = d_al + (tw ? cB * N : 0);
+    double* d_ga = d_be + (tw ? cB * N : 0);
+    double* d_sc = d_ga + (tw ? cB * N : 0);  // 5 x [cB] scalars, each slot padded to 2*... keep 16B aligned
+    const size_t sc_stride = (cB + 1) & ~(size_t)1;
+    // copies of chunk `it` wait until the kernels that last used this buffer are done
+    if (it >= 2) LISA_CUDA(cudaStreamWaitEvent(p->s_copy, p->done[buf], 0));
+#define H2D(dst, src, count) LISA_CUDA(cudaMemcpyAsync((dst), (src), sizeof(double) * (count), cudaMemcpyHostToDevice, p->s_copy))
+    H2D(d_amp, amp_host + (size_t)b0 * M * N, nb * M * N);
+    H2D(d_pha, phase_host + (size_t)b0 * M * N, nb * M * N);
+    if (tw) {
+      H2D(d_al, alpha_host + (size_t)b0 * N, nb * N);
+      H2D(d_be, beta_host + (size_t)b0 * N, nb * N);
+      H2D(d_ga, gamma_host + (size_t)b0 * N, nb * N);
+    }
+    H2D(d_sc + 0 * sc_stride, iota_host + b0, nb);
+    H2D(d_sc + 1 * sc_stride, phi_host + b0, nb);
+    H2D(d_sc + 2 * sc_stride, psi_host + b0, nb);
+    H2D(d_sc + 3 * sc_stride, lambda_host + b0, nb);
+    H2D(d_sc + 4 * sc_stride, beta_sky_host + b0, nb);
+#undef H2D
+    LISA_CUDA(cudaEventRecord(p->copied[buf], p->s_copy));
+    LISA_CUDA(cudaStreamWaitEvent(p->s_comp, p->copied[buf], 0));
+    if ((rc = run_modes_to_pol((int)nb, N, n_modes, l_host, m_host, d_amp, d_pha, tw ? d_al : nullptr,
+                               tw ? d_be : nullptr, tw ? d_ga : nullptr, d_sc, d_sc + sc_stride,
+                               d_sc + 2 * sc_stride, nullptr, p->hp, p->hc, p->s_comp)))
+      return rc;
+    if ((rc = run_link_response((int)nb, N, t0, dt, order, margin_y, p->hp, p->hc, d_sc + 3 * sc_stride,
+                                d_sc + 4 * sc_stride, od, p->y, p->s_comp)))
+      return rc;
+    if ((rc = run_tdi((int)nb, N, t0, dt, order, generation, 1, margin_lo, margin_hi, p->y, od, p->tdi, p->s_comp)))
+      return rc;
+    if ((rc = run_loglike(p->plan, (int)nb, N, p->tdi, p->data_spec, p->weight, kmin, kmax, p->ll, p->ll + sc_stride,
+                          p->ll + 2 * sc_stride, p->s_comp)))
+      return rc;
+    LISA_CUDA(cudaMemcpyAsync(loglike_host + b0, p->ll, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));
+    if (dh_host) LISA_CUDA(cudaMemcpyAsync(dh_host + b0, p->ll + sc_stride, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));
+    if (hh_host) LISA_CUDA(cudaMemcpyAsync(hh_host + b0, p->ll + 2 * sc_stride, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));
+    LISA_CUDA(cudaEventRecord(p->done[buf], p->s_comp));
+  }
+  LISA_CUDA(cudaStreamSynchronize(p->s_copy));
+  LISA_CUDA(cudaStreamSynchronize(p->s_comp));
+  return LISA_TD_OK;
+}
+
+// ---------------------------------------------------------------------- DFMA probe
+__global__ void k_probe_dfma(long long iters, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3;
+  double a4 = a0 + 4e-3, a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.999999, c = 1e-7;
+  for (long long i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+int lisa_td_probe_dfma(long long iters, int blocks, int threads, double* sink, float* ms_host, void* stream) {
+  const char* fn = "lisa_td_probe_dfma";
+  if (iters <= 0 || blocks <= 0 || threads <= 0 || threads > 1024 || !sink || !ms_host)
+    return set_error(LISA_TD_EINVAL, "%s: bad arguments", fn);
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0, e1;
+  LISA_CUDA(cudaEventCreate(&e0));
+  LISA_CUDA(cudaEventCreate(&e1));
+  LISA_CUDA(cudaEventRecord(e0, st));
+  k_probe_dfma<<<blocks, threads, 0, st>>>(iters, sink);
+  LISA_CUDA(cudaPeekAtLastError());
+  LISA_CUDA(cudaEventRecord(e1, st));
+  LISA_CUDA(cudaEventSynchronize(e1));
+  LISA_CUDA(cudaEventElapsedTime(ms_host, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return LISA_TD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,237 @@
+// common.cuh -- shared device/host helpers of liblisa_td (sm_100a only).
+//
+// Nothing in this directory includes, links or reads anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lisa_td.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "liblisa_td is written for sm_100a (B200) only"
+#endif
+
+namespace lisa {
+
+// ------------------------------------------------------------------ errors (api.cu)
+int set_error(int code, const char* fmt, ...);
+int check_cuda(cudaError_t e, const char* what);
+#define LISA_CUDA(call)                                        \
+  do {                                                         \
+    int _rc = ::lisa::check_cuda((call), #call);               \
+    if (_rc != LISA_TD_OK) return _rc;                         \
+  } while (0)
+#define LISA_LAUNCH_CHECK(name) LISA_CUDA(cudaPeekAtLastError())
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+constexpr double C_LIGHT = 299792458.0;  // m/s
+constexpr int MAX_HALF = 32;             // (p+1)/2 for p <= 63
+
+// ------------------------------------------------------------------ Lagrange weights
+// Taps j = -H+1 .. H (H = (p+1)/2).  Nodes are paired (k, 1-k), k = 1..H:
+//   (eps-k)(eps-(1-k)) = eps(eps-1) + k(1-k),
+// and the barycentric weights satisfy w_{1-k} = -w_k,  w_k = (-1)^{H-k} / ((k+H-1)! (H-k)!).
+// w[k-1] holds w_k, computed on the host in long double.  Passed to kernels BY VALUE so it
+// lands in the constant bank (no global state, no races between streams).
+struct LagW {
+  double w[MAX_HALF];
+};
+void make_lagw(int order, LagW* out);
+
+// ------------------------------------------------------------------ orbit (device form)
+// KEPLER1 is evaluated as  r_k(t) = a (cos M, sin M, 0) + delta_k(t)  with the common 1 AU
+// part split off ALGEBRAICALLY (exact rearrangement of reading A8), so that arm vectors and
+// the differential delays between spacecraft are formed from ~1e9 m quantities rather than
+// as differences of 1.5e11 m ones ("delay arithmetic").
+struct OrbitDev {
+  int kind;
+  double w, t_ref, phase0;        // mean motion 2 pi / year
+  double a, a_over_c;             // semi-major axis [m], [s]
+  double e, ci, si, dci, bq, dbq; // eccentricity, cos/sin inclination, ci-1, sqrt(1-e^2), bq-1
+  double cs[3], sn[3];            // cos/sin of sigma_k = 2 pi k / 3
+  double r[3][3];                 // STATIC positions [m]
+  double L[6];                    // STATIC light travel times [s]
+  double max_r_over_c;            // host-side bounds used for margin validation [s]
+  double max_L;                   // [s]
+};
+int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* out);
+
+#ifdef __CUDACC__
+
+// Link index 0..5 <-> l = [1,2,3,-1,-2,-3]; sender / receiver spacecraft (0-based).
+__host__ __device__ constexpr int link_s(int l) { return l < 3 ? (l + 2) % 3 : (l - 3 + 1) % 3; }
+__host__ __device__ constexpr int link_r(int l) { return l < 3 ? (l + 1) % 3 : (l - 3 + 2) % 3; }
+
+// ------------------------------------------------------------------ sincos
+// fp64 sin/cos with a two-constant Cody-Waite reduction done with FMAs.  x - k*PIO2_HI is
+// exact (both are multiples of 2^-52 and the result is < 1), the second FMA rounds once, and
+// the neglected tail of pi/2 is 1.5e-33*k, so the reduced argument is good to ~6e-17 for any
+// |x| < 2^30 -- no Payne-Hanek slow path for the 1e5..1e6 rad phases of a months-long chirp.
+// Kernels: Taylor polynomials on |r| <= pi/4 (remainders 8e-20 and 2e-18).
+__device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
+  const double TWO_OVER_PI = 0.6366197723675814;
+  const double PIO2_HI = 1.5707963267948966;
+  const double PIO2_LO = 6.123233995736766e-17;
+  double kd = rint(x * TWO_OVER_PI);
+  int q = __double2int_rn(kd);
+  double r = fma(-kd, PIO2_HI, x);
+  r = fma(-kd, PIO2_LO, r);
+  double r2 = r * r;
+  // sin r = r + r^3 (-1/3! + r^2/5! - ... + r^14/17!)
+  double ps = 2.8114572543455206e-15;
+  ps = fma(ps, r2, -7.647163731819816e-13);
+  ps = fma(ps, r2, 1.6059043836821613e-10);
+  ps = fma(ps, r2, -2.505210838544172e-08);
+  ps = fma(ps, r2, 2.7557319223985893e-06);
+  ps = fma(ps, r2, -0.0001984126984126984);
+  ps = fma(ps, r2, 0.008333333333333333);
+  ps = fma(ps, r2, -0.16666666666666666);
+  double sr = fma(ps * r2, r, r);
+  // cos r = 1 - r^2/2 + r^4 (1/4! - r^2/6! + ... + r^12/16!)
+  double pc = 4.779477332387385e-14;
+  pc = fma(pc, r2, -1.1470745597729725e-11);
+  pc = fma(pc, r2, 2.08767569878681e-09);
+  pc = fma(pc, r2, -2.755731922398589e-07);
+  pc = fma(pc, r2, 2.48015873015873e-05);
+  pc = fma(pc, r2, -0.001388888888888889);
+  pc = fma(pc, r2, 0.041666666666666664);
+  double cr = fma(pc * r2, r2, fma(-0.5, r2, 1.0));
+  double ss = (q & 1) ? cr : sr;
+  double cc = (q & 1) ? sr : cr;
+  s = (q & 2) ? -ss : ss;
+  c = ((q + 1) & 2) ? -cc : cc;
+}
+
+// ------------------------------------------------------------------ orbit evaluation
+// delta[k][xyz]: spacecraft positions minus the common part a(cM, sM, 0)  (STATIC: the
+// positions themselves, cM = sM = 0).
+__device__ __forceinline__ void orbit_offsets(const OrbitDev& o, double t, double (&d)[3][3],
+                                              double& cM, double& sM) {
+  if (o.kind == 0) {
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) d[k][j] = o.r[k][j];
+    cM = 0.0;
+    sM = 0.0;
+    return;
+  }
+  double M = fma(o.w, t - o.t_ref, -o.phase0);
+  sincos_d(M, sM, cM);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    // M_k = M - sigma_k
+    double cMk = fma(cM, o.cs[k], sM * o.sn[k]);
+    double sMk = fma(sM, o.cs[k], -cM * o.sn[k]);
+    // psi_k = M_k + s, s = e sin M_k;  cos psi_k = cMk + dc, sin psi_k = sMk + ds
+    double s = o.e * sMk, sh, ch;
+    sincos_d(0.5 * s, sh, ch);
+    double sins = 2.0 * sh * ch, cosm1 = -2.0 * sh * sh;
+    double dc = fma(cMk, cosm1, -sMk * sins);
+    double ds = fma(sMk, cosm1, cMk * sins);
+    double u1 = dc - o.e;
+    double px = fma(o.dci, cMk, o.ci * u1);  // x/a - cos M_k
+    double py = fma(o.dbq, sMk, o.bq * ds);  // y/a - sin M_k
+    d[k][0] = o.a * fma(o.cs[k], px, -o.sn[k] * py);
+    d[k][1] = o.a * fma(o.sn[k], px, o.cs[k] * py);
+    d[k][2] = o.a * o.si * (cMk + u1);
+  }
+}
+
+// Light travel times of the six links at time t (link order [1,2,3,-1,-2,-3]).
+__device__ __forceinline__ void orbit_arm_times(const OrbitDev& o, double t, double (&L)[6]) {
+  if (o.kind == 0) {
+#pragma unroll
+    for (int l = 0; l < 6; ++l) L[l] = o.L[l];
+    return;
+  }
+  double d[3][3], cM, sM;
+  orbit_offsets(o, t, d, cM, sM);
+#pragma unroll
+  for (int l = 0; l < 3; ++l) {
+    const int s = (l + 2) % 3, r = (l + 1) % 3;  // link l+1: sender, receiver
+    double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
+    double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) / C_LIGHT;
+    L[l] = len;
+    L[l + 3] = len;
+  }
+}
+
+// ------------------------------------------------------------------ Lagrange stencil
+// HT > 0: half-width known at compile time (fully unrolled, prefix products in registers).
+// HT = 0: runtime half-width Hrt <= MAX_HALF (prefix products in local memory).
+//
+// lagrange_coeffs: c[j + H - 1] = c_j(eps), j = -H+1..H.   ~9 fp64 ops per node pair.
+template <int HT>
+__device__ __forceinline__ void lagrange_coeffs(double eps, int Hrt, const LagW& lw,
+                                                double* __restrict__ c) {
+  const int H = HT > 0 ? HT : Hrt;
+  double P[HT > 0 ? HT + 1 : MAX_HALF + 1];
+  const double q = eps * (eps - 1.0);
+  P[1] = 1.0;
+#pragma unroll
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
+  double S = 1.0;
+#pragma unroll
+  for (int k = H; k >= 1; --k) {
+    double a = (lw.w[k - 1] * P[k]) * S;
+    c[k + H - 1] = a * (eps + (double)(k - 1));
+    c[H - k] = a * ((double)k - eps);
+    S *= q + (double)(k * (1 - k));
+  }
+}
+
+// Fused coefficient sweep + dot product with an interleaved (h+, hx) series:
+// x points at tap j = 0, i.e. x[j] is read for j = -H+1..H.
+template <int HT>
+__device__ __forceinline__ void lagrange_dot2(double eps, int Hrt, const LagW& lw,
+                                              const double2* __restrict__ x, double& sp,
+                                              double& sc) {
+  const int H = HT > 0 ? HT : Hrt;
+  double P[HT > 0 ? HT + 1 : MAX_HALF + 1];
+  const double q = eps * (eps - 1.0);
+  P[1] = 1.0;
+#pragma unroll
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
+  double S = 1.0, ap = 0.0, ac = 0.0, bp = 0.0, bc = 0.0;
+#pragma unroll
+  for (int k = H; k >= 1; --k) {
+    double a = (lw.w[k - 1] * P[k]) * S;
+    double ck = a * (eps + (double)(k - 1));
+    double cm = a * ((double)k - eps);
+    double2 xk = x[k], xm = x[1 - k];
+    ap = fma(ck, xk.x, ap);
+    ac = fma(ck, xk.y, ac);
+    bp = fma(cm, xm.x, bp);
+    bc = fma(cm, xm.y, bc);
+    S *= q + (double)(k * (1 - k));
+  }
+  sp = ap + bp;
+  sc = ac + bc;
+}
+
+// Same for a single series.
+template <int HT>
+__device__ __forceinline__ double lagrange_dot1(double eps, int Hrt, const LagW& lw,
+                                                const double* __restrict__ x) {
+  const int H = HT > 0 ? HT : Hrt;
+  double P[HT > 0 ? HT + 1 : MAX_HALF + 1];
+  const double q = eps * (eps - 1.0);
+  P[1] = 1.0;
+#pragma unroll
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
+  double S = 1.0, a0 = 0.0, a1 = 0.0;
+#pragma unroll
+  for (int k = H; k >= 1; --k) {
+    double a = (lw.w[k - 1] * P[k]) * S;
+    a0 = fma(a * (eps + (double)(k - 1)), x[k], a0);
+    a1 = fma(a * ((double)k - eps), x[1 - k], a1);
+    S *= q + (double)(k * (1 - k));
+  }
+  return a0 + a1;
+}
+
+#endif  // __CUDACC__
+
+}  // namespace lisa

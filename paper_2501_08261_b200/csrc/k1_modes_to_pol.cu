@@ -1,0 +1,216 @@
+// k1_modes_to_pol.cu -- S1: co-precessing modes -> h+, hx by the paper's single-sum form
+// (Eq. 2.4-2.6) with readings A1-A6 of DESIGN.md:
+//
+//   h+ - i hx = e^{2 i psi} sum_modes N_l [ h_lm frakD^l_{m,2}(Q) + (-1)^l conj(h_lm) frakD^l_{-m,2}(Q) ],
+//   h_lm = amp e^{-i phase},  N_l = sqrt((2l+1)/4pi),
+//   Q = Q(alpha,beta,gamma)(t) * Q(euler0) * Q(phi, iota, 0)          (one composed rotation),
+//   Q(a,b,g) = (Qa, Qb) = (cos(b/2) e^{i(a+g)/2}, sin(b/2) e^{-i(a-g)/2})   (Eq. 2.5 / sqrt 2, A3).
+//
+// Eq. 2.6 (with A4) is used in its division-free polynomial form (A5): for row m' and column 2
+//   frakD^l_{m',2} = PA(m'+2) PB(2-m') sum_rho coef_rho A^{eA0-i} B^{eB0+i},  A=|Qa|^2, B=|Qb|^2,
+//   PA(k) = Qa^k (k>=0) or conj(Qa)^{-k},   PB(k) = Qb^k or conj(Qb)^{-k},
+// so nothing is divided by |Qa|^2 when the total beta reaches pi.  The host turns the mode
+// list into such "rows" (two per mode, one for m = 0); the kernel evaluates them.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace lisa {
+
+constexpr int K1_MAX_MODES = 16;
+constexpr int K1_MAX_ROWS = 2 * K1_MAX_MODES;
+constexpr int K1_MAX_TERMS = 7;  // rho range of column 2 for l <= 8
+constexpr int K1_PMAX = 10;      // largest power of Qa / Qb: l + 2
+constexpr int K1_EMAX = 8;       // largest power of A / B
+constexpr int K1_THREADS = 256;
+constexpr int K1_PER_THREAD = 4;
+
+struct K1Row {
+  short mode, conj, ka, kb, eA0, eB0, nterms, pad;
+  double coef[K1_MAX_TERMS];
+};
+struct K1Params {
+  int B;
+  long long N;
+  int n_modes, n_rows, twisted, have_e0;
+  const double *amp, *phase, *alpha, *beta, *gamma, *iota, *phi, *psi, *euler0;
+  double *hplus, *hcross;
+  K1Row row[K1_MAX_ROWS];
+};
+
+struct cplx {
+  double re, im;
+};
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return {fma(a.re, b.re, -a.im * b.im), fma(a.re, b.im, a.im * b.re)};
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return {a.re, -a.im}; }
+
+struct quat {
+  cplx a, b;
+};
+__device__ __forceinline__ quat quat_from_euler(double al, double be, double ga) {
+  double sb, cb, sp, cp, sm, cm;
+  sincos_d(0.5 * be, sb, cb);
+  sincos_d(0.5 * (al + ga), sp, cp);
+  sincos_d(0.5 * (al - ga), sm, cm);
+  return {{cb * cp, cb * sp}, {sb * cm, -sb * sm}};
+}
+// consecutive rotations R_p R_q:  (pa qa - conj(pb) qb,  pb qa + conj(pa) qb)
+__device__ __forceinline__ quat quat_mul(quat p, quat q) {
+  cplx t1 = cmul(p.a, q.a), t2 = cmul(cconj(p.b), q.b);
+  cplx t3 = cmul(p.b, q.a), t4 = cmul(cconj(p.a), q.b);
+  return {{t1.re - t2.re, t1.im - t2.im}, {t3.re + t4.re, t3.im + t4.im}};
+}
+
+struct PowTables {
+  cplx qa[K1_PMAX + 1], qb[K1_PMAX + 1];
+  double A[K1_EMAX + 1], B[K1_EMAX + 1];
+};
+__device__ __forceinline__ void build_tables(const quat& Q, PowTables& T) {
+  T.qa[0] = {1.0, 0.0};
+  T.qb[0] = {1.0, 0.0};
+  T.A[0] = 1.0;
+  T.B[0] = 1.0;
+  const double A = fma(Q.a.re, Q.a.re, Q.a.im * Q.a.im);
+  const double B = fma(Q.b.re, Q.b.re, Q.b.im * Q.b.im);
+#pragma unroll
+  for (int k = 1; k <= K1_PMAX; ++k) {
+    T.qa[k] = cmul(T.qa[k - 1], Q.a);
+    T.qb[k] = cmul(T.qb[k - 1], Q.b);
+  }
+#pragma unroll
+  for (int k = 1; k <= K1_EMAX; ++k) {
+    T.A[k] = T.A[k - 1] * A;
+    T.B[k] = T.B[k - 1] * B;
+  }
+}
+// N_l (+-)^l frakD^l_{m',2}(Q) of one row
+__device__ __forceinline__ cplx row_weight(const K1Row& r, const PowTables& T) {
+  cplx pa = r.ka >= 0 ? T.qa[r.ka] : cconj(T.qa[-r.ka]);
+  cplx pb = r.kb >= 0 ? T.qb[r.kb] : cconj(T.qb[-r.kb]);
+  double poly = 0.0;
+  for (int i = 0; i < r.nterms; ++i) poly = fma(r.coef[i], T.A[r.eA0 - i] * T.B[r.eB0 + i], poly);
+  cplx w = cmul(pa, pb);
+  return {w.re * poly, w.im * poly};
+}
+
+__global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol(const K1Params p) {
+  __shared__ quat Qc;             // Q(euler0) * Q(phi, iota, 0) of this walker
+  __shared__ double rot[2];       // cos 2 psi, sin 2 psi
+  __shared__ cplx Wc[K1_MAX_ROWS];  // aligned-spin case: constant row weights
+  const int b = blockIdx.y;
+  if (threadIdx.x == 0) {
+    quat q = quat_from_euler(p.phi[b], p.iota[b], 0.0);  // footnote 1
+    if (p.have_e0)
+      q = quat_mul(quat_from_euler(p.euler0[3 * b], p.euler0[3 * b + 1], p.euler0[3 * b + 2]), q);
+    Qc = q;
+    double s2, c2;
+    sincos_d(2.0 * p.psi[b], s2, c2);
+    rot[0] = c2;
+    rot[1] = s2;
+  }
+  __syncthreads();
+  if (!p.twisted) {
+    if (threadIdx.x < p.n_rows) {
+      PowTables T;
+      build_tables(Qc, T);
+      Wc[threadIdx.x] = row_weight(p.row[threadIdx.x], T);
+    }
+    __syncthreads();
+  }
+  const size_t bN = (size_t)b * p.N;
+  const double* amp = p.amp + bN * p.n_modes;
+  const double* pha = p.phase + bN * p.n_modes;
+  const long long n_base = (long long)blockIdx.x * (K1_THREADS * K1_PER_THREAD);
+  for (int it = 0; it < K1_PER_THREAD; ++it) {
+    const long long n = n_base + it * K1_THREADS + threadIdx.x;
+    if (n >= p.N) break;
+    PowTables T;
+    if (p.twisted) {
+      quat q = quat_mul(quat_from_euler(p.alpha[bN + n], p.beta[bN + n], p.gamma[bN + n]), Qc);
+      build_tables(q, T);
+    }
+    double Hre = 0.0, Him = 0.0;
+    for (int r = 0; r < p.n_rows; ++r) {
+      const K1Row& row = p.row[r];
+      const int k = row.mode;
+      // rows of one mode are adjacent; the sincos is recomputed only when the mode changes
+      double s, c;
+      const double a = amp[(size_t)k * p.N + n];
+      sincos_d(pha[(size_t)k * p.N + n], s, c);
+      // h = a (c - i s);  conj row uses a (c + i s)
+      const double hre = a * c, him = row.conj ? a * s : -a * s;
+      cplx w = p.twisted ? row_weight(row, T) : Wc[r];
+      Hre += fma(hre, w.re, -him * w.im);
+      Him += fma(hre, w.im, him * w.re);
+      if (r + 1 < p.n_rows && p.row[r + 1].mode == k) {  // the -m partner: reuse a, s, c
+        ++r;
+        const K1Row& row2 = p.row[r];
+        const double him2 = row2.conj ? a * s : -a * s;
+        cplx w2 = p.twisted ? row_weight(row2, T) : Wc[r];
+        Hre += fma(hre, w2.re, -him2 * w2.im);
+        Him += fma(hre, w2.im, him2 * w2.re);
+      }
+    }
+    // e^{2 i psi};  h+ = Re H, hx = -Im H
+    p.hplus[bN + n] = fma(Hre, rot[0], -Him * rot[1]);
+    p.hcross[bN + n] = -fma(Hre, rot[1], Him * rot[0]);
+  }
+}
+
+static double factorial_ld(int n) {
+  long double f = 1;
+  for (int i = 2; i <= n; ++i) f *= i;
+  return (double)f;
+}
+static long double binom_ld(int n, int k) {
+  if (k < 0 || k > n) return 0;
+  long double r = 1;
+  for (int i = 1; i <= k; ++i) r = r * (n - k + i) / i;
+  return r;
+}
+
+int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m, const double* amp,
+                     const double* phase, const double* alpha, const double* beta,
+                     const double* gamma, const double* iota, const double* phi,
+                     const double* psi, const double* euler0, double* hplus, double* hcross,
+                     cudaStream_t st) {
+  K1Params p;
+  p.B = B; p.N = N; p.n_modes = n_modes; p.twisted = alpha != nullptr; p.have_e0 = euler0 != nullptr;
+  p.amp = amp; p.phase = phase; p.alpha = alpha; p.beta = beta; p.gamma = gamma;
+  p.iota = iota; p.phi = phi; p.psi = psi; p.euler0 = euler0; p.hplus = hplus; p.hcross = hcross;
+  int nr = 0;
+  const long double PI_L = 3.14159265358979323846264338327950288L;
+  for (int k = 0; k < n_modes; ++k) {
+    const int ll = l[k], mm = m[k];
+    for (int sgn = +1; sgn >= -1; sgn -= 2) {
+      if (sgn < 0 && mm == 0) break;
+      const int mp = sgn * mm;
+      K1Row& r = p.row[nr++];
+      r.mode = (short)k; r.conj = sgn < 0; r.ka = (short)(mp + 2); r.kb = (short)(2 - mp); r.pad = 0;
+      const int rmin = mp - 2 > 0 ? mp - 2 : 0;
+      const int rmax = (ll + mp < ll - 2) ? ll + mp : ll - 2;
+      r.eA0 = (short)(r.ka >= 0 ? ll - 2 - rmin : ll + mp - rmin);
+      r.eB0 = (short)(r.kb >= 0 ? rmin : rmin - (mp - 2));
+      r.nterms = (short)(rmax - rmin + 1);
+      const long double pref = sqrtl((long double)factorial_ld(ll + 2) * factorial_ld(ll - 2) /
+                                     ((long double)factorial_ld(ll + mp) * factorial_ld(ll - mp)));
+      const long double norm = sqrtl((2 * ll + 1) / (4 * PI_L));
+      for (int i = 0; i < K1_MAX_TERMS; ++i) r.coef[i] = 0.0;
+      for (int rho = rmin; rho <= rmax; ++rho) {
+        long double c = binom_ld(ll + mp, rho) * binom_ld(ll - mp, ll - rho - 2) * pref * norm;
+        if (rho & 1) c = -c;
+        if (sgn < 0 && (ll & 1)) c = -c;  // h_{l,-m} = (-1)^l conj(h_lm)  (A6)
+        r.coef[rho - rmin] = (double)c;
+      }
+    }
+  }
+  p.n_rows = nr;
+  dim3 grid((unsigned)((N + K1_THREADS * K1_PER_THREAD - 1) / (K1_THREADS * K1_PER_THREAD)), (unsigned)B);
+  k1_modes_to_pol<<<grid, K1_THREADS, 0, st>>>(p);
+  LISA_LAUNCH_CHECK("k1_modes_to_pol");
+  return LISA_TD_OK;
+}
+
+}  // namespace lisa

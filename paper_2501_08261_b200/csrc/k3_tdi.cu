@@ -1,0 +1,332 @@
+// k3_tdi.cu -- S3: six links -> TDI X,Y,Z (generation 1.5 / 2) -> A,E,T
+// (Eq. 2.9-2.11; readings A9, A10 of DESIGN.md).
+//
+// The delays of TDI are sums of light travel times L_l(t_n): they depend on time but NOT on
+// the walker.  The fast kernel therefore gives one block a tile of 32 output samples and ALL
+// walkers: each thread (sample, channel x series) first merges the 4 (generation 2) or 2
+// (generation 1.5) delayed reads that hit its y series into ONE stencil of WIN taps held in
+// registers (the interpolation is linear in y, so  sum_t s_t sum_j c_j(eps_t) y[n-K_t+j]  =
+// sum_i C_i y[n+LOW+i]), then streams the walkers through shared memory (cp.async, double
+// buffered) doing WIN FMAs per walker.  48 coefficient sets per output sample are thus paid
+// once per tile instead of once per walker, and 16x32 taps shrink to 4xWIN.
+//
+// A plain one-thread-per-(walker, sample) kernel covers every other order / cadence.
+#include "common.cuh"
+
+namespace lisa {
+
+struct K3Term {
+  signed char sign;
+  signed char mult[6];  // multiplicity of each L_l in the delay
+  signed char pad;
+};
+struct K3Pair {
+  int series;   // link index 0..5 of the y series
+  int n_terms;  // 4 (generation 2) or 2 (generation 1.5)
+  K3Term t[4];
+};
+struct K3Params {
+  int B;
+  long long N;
+  double t0, dt, inv_dt;
+  int half, generation, out_kind, kcap;
+  long long margin_lo, margin_hi;
+  const double* y;
+  double* tdi;
+  OrbitDev orb;
+  LagW lw;
+  K3Pair pair[12];  // [channel X,Y,Z][slot]
+};
+
+// ---- term tables, restated from the paper ----------------------------------------------
+// Michelson X, one line per y series: "link : sign {delay labels}" (labels are signed link
+// numbers, each standing for one light travel time L_label).
+// Eq. 2.9:
+//   y_{1-32} = link -3 : +{3,2,-2}  -{3}
+//   y_{231}  = link  3 : +{2,-2}    -{}
+//   y_{123}  = link  2 : +{-2}      -{-2,-3,3}
+//   y_{3-21} = link -2 : +{}        -{-3,3}
+// Eq. 2.10 adds, per series, the same two terms delayed by a further
+// L2+L-2+L3+L-3 with opposite sign (y123 block per reading A9).
+struct TermSpec {
+  int link;
+  int sign;
+  int n;
+  int d[7];
+};
+static const TermSpec kX15[8] = {
+    {-3, +1, 3, {3, 2, -2}},  {-3, -1, 1, {3}},
+    {3, +1, 2, {2, -2}},      {3, -1, 0, {}},
+    {2, +1, 1, {-2}},         {2, -1, 3, {-2, -3, 3}},
+    {-2, +1, 0, {}},          {-2, -1, 2, {-3, 3}},
+};
+static const TermSpec kX20extra[8] = {
+    {-3, +1, 5, {-2, 2, 3, 3, -3}},         {-3, -1, 7, {3, 3, -3, -2, -2, 2, 2}},
+    {3, +1, 4, {-2, 2, 3, -3}},             {3, -1, 6, {3, -3, -2, -2, 2, 2}},
+    {2, +1, 7, {-2, -2, 2, 3, 3, -3, -3}},  {2, -1, 5, {3, -3, -2, -2, 2}},
+    {-2, +1, 6, {-2, 2, 3, 3, -3, -3}},     {-2, -1, 4, {3, -3, -2, 2}},
+};
+
+static int cyc_label(int label, int times) {  // 1->2->3->1 on |label|, sign kept
+  int s = label < 0 ? -1 : 1, a = label < 0 ? -label : label;
+  for (int i = 0; i < times; ++i) a = a % 3 + 1;
+  return s * a;
+}
+static int label_index(int label) { return label > 0 ? label - 1 : -label + 2; }
+
+static void build_pairs(int generation, K3Pair* out) {
+  for (int c = 0; c < 3; ++c)
+    for (int slot = 0; slot < 4; ++slot) {
+      K3Pair& pr = out[c * 4 + slot];
+      pr.series = label_index(cyc_label(kX15[2 * slot].link, c));
+      pr.n_terms = 0;
+      for (int pass = 0; pass < (generation == 20 ? 2 : 1); ++pass)
+        for (int k = 0; k < 2; ++k) {
+          const TermSpec& ts = pass == 0 ? kX15[2 * slot + k] : kX20extra[2 * slot + k];
+          K3Term& t = pr.t[pr.n_terms++];
+          t.sign = (signed char)ts.sign;
+          t.pad = 0;
+          for (int i = 0; i < 6; ++i) t.mult[i] = 0;
+          for (int i = 0; i < ts.n; ++i) t.mult[label_index(cyc_label(ts.d[i], c))]++;
+        }
+      for (int k = pr.n_terms; k < 4; ++k) {
+        pr.t[k].sign = 0;
+        pr.t[k].pad = 0;
+        for (int i = 0; i < 6; ++i) pr.t[k].mult[i] = 0;
+      }
+    }
+}
+
+__device__ __forceinline__ double term_delay(const K3Term& t, const double (&L)[6], double inv_dt) {
+  double D = 0.0;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) D = fma((double)t.mult[i], L[i], D);
+  return D * inv_dt;
+}
+
+__device__ __forceinline__ void combine_out(int out_kind, double X, double Y, double Z, double (&o)[3]) {
+  if (out_kind == 0) {
+    o[0] = X; o[1] = Y; o[2] = Z;
+  } else {  // Eq. 2.11
+    o[0] = (Z - X) * 0.70710678118654752440;
+    o[1] = (X - 2.0 * Y + Z) * 0.40824829046386301637;
+    o[2] = (X + Y + Z) * 0.57735026918962576451;
+  }
+}
+
+// ---------------------------------------------------------------- generic kernel
+__global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
+  const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (n >= p.N) return;
+  double* ob = p.tdi + (size_t)b * 3 * p.N;
+  if (n < p.margin_lo || n >= p.N - p.margin_hi) {
+    for (int c = 0; c < 3; ++c) ob[(size_t)c * p.N + n] = 0.0;
+    return;
+  }
+  const double* yb = p.y + (size_t)b * 6 * p.N;
+  double L[6];
+  orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
+  double xyz[3];
+  for (int c = 0; c < 3; ++c) {
+    double acc = 0.0;
+    for (int s = 0; s < 4; ++s) {
+      const K3Pair& pr = p.pair[c * 4 + s];
+      const double* ser = yb + (size_t)pr.series * p.N;
+      for (int k = 0; k < pr.n_terms; ++k) {
+        const double D = term_delay(pr.t[k], L, p.inv_dt);
+        const double Kf = ceil(D);
+        const double eps = Kf - D;
+        long long base = n - (long long)Kf;
+        base = max((long long)(p.half - 1), min(base, p.N - 1 - p.half));
+        acc += (double)pr.t[k].sign * lagrange_dot1<0>(eps, p.half, p.lw, ser + base);
+      }
+    }
+    xyz[c] = acc;
+  }
+  double o[3];
+  combine_out(p.out_kind, xyz[0], xyz[1], xyz[2], o);
+  for (int c = 0; c < 3; ++c) ob[(size_t)c * p.N + n] = o[c];
+}
+
+// ---------------------------------------------------------------- merged-stencil kernel
+constexpr int K3_TS = 32;       // output samples per block (one warp lane each)
+constexpr int K3_PAIRS = 12;    // warps per block: channel x series
+constexpr int K3_THREADS = K3_TS * K3_PAIRS;
+constexpr int K3_WC = 8;        // walkers per shared-memory chunk
+
+__device__ __forceinline__ void cp_async8_zfill(void* smem, const void* gmem, bool valid) {
+  unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  int sz = valid ? 8 : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(sa), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int NKEEP>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP));
+}
+
+// Adds sgn * c_j(eps) into the merged stencil at compile-time offset OFF.
+template <int H, int WIN, int OFF>
+__device__ __forceinline__ void add_term_at(double (&C)[WIN], double eps, double sgn, const LagW& lw) {
+  double P[H + 1];
+  const double q = eps * (eps - 1.0);
+  P[1] = 1.0;
+#pragma unroll
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
+  double S = sgn;
+#pragma unroll
+  for (int k = H; k >= 1; --k) {
+    double a = (lw.w[k - 1] * P[k]) * S;
+    C[OFF + k + H - 1] = fma(a, eps + (double)(k - 1), C[OFF + k + H - 1]);
+    C[OFF + H - k] = fma(a, (double)k - eps, C[OFF + H - k]);
+    S *= q + (double)(k * (1 - k));
+  }
+}
+template <int H, int WIN, int OFF>
+struct TermDispatch {
+  static __device__ __forceinline__ void run(double (&C)[WIN], int off, double eps, double sgn, const LagW& lw) {
+    if (off == OFF) add_term_at<H, WIN, OFF>(C, eps, sgn, lw);
+    else TermDispatch<H, WIN, OFF - 1>::run(C, off, eps, sgn, lw);
+  }
+};
+template <int H, int WIN>
+struct TermDispatch<H, WIN, -1> {
+  static __device__ __forceinline__ void run(double (&)[WIN], int, double, double, const LagW&) {}
+};
+
+template <int H, int WIN>
+__global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_merged(const K3Params p) {
+  constexpr int KCAP = WIN - 2 * H;       // largest integer delay the window can hold
+  constexpr int TW = K3_TS + WIN - 1;     // y samples per row of the tile
+  constexpr int LOW = -(KCAP + H - 1);    // offset of stencil tap 0 relative to n
+  extern __shared__ double smem[];
+  double* ys = smem;                                   // [2][WC][6][TW]
+  double* red = smem + 2 * K3_WC * 6 * TW;             // [WC][12][32]
+  const int lane = threadIdx.x & 31;
+  const int pr_id = threadIdx.x >> 5;
+  const long long n0 = (long long)blockIdx.x * K3_TS;
+  const long long n = n0 + lane;
+
+  // ---- phase 1: merged stencil of my (channel, series) pair at my sample, in registers
+  double C[WIN];
+#pragma unroll
+  for (int i = 0; i < WIN; ++i) C[i] = 0.0;
+  const K3Pair& pr = p.pair[pr_id];
+  if (n >= p.margin_lo && n < p.N - p.margin_hi) {
+    double L[6];
+    orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
+    for (int k = 0; k < pr.n_terms; ++k) {
+      const double D = term_delay(pr.t[k], L, p.inv_dt);
+      const double Kf = ceil(D);
+      const double eps = Kf - D;
+      int off = KCAP - (int)Kf;
+      off = max(0, min(off, KCAP));
+      TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.lw);
+    }
+  }
+  const int series = pr.series;
+
+  // ---- phase 2: stream walkers
+  const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
+  auto prefetch = [&](int chunk, int buf) {
+    double* dst = ys + (size_t)buf * K3_WC * 6 * TW;
+    for (int e = threadIdx.x; e < K3_WC * 6 * TW; e += K3_THREADS) {
+      const int row = e / TW, i = e - row * TW;
+      const int w = chunk * K3_WC + row / 6;
+      const long long g = n0 + LOW + i;
+      const bool ok = (w < p.B) && g >= 0 && g < p.N;
+      const size_t src = ok ? ((size_t)w * 6 + (row % 6)) * p.N + g : 0;
+      cp_async8_zfill(dst + e, p.y + src, ok);
+    }
+    cp_async_commit();
+  };
+  prefetch(0, 0);
+  for (int ch = 0; ch < n_chunks; ++ch) {
+    const int buf = ch & 1;
+    if (ch + 1 < n_chunks) {
+      prefetch(ch + 1, buf ^ 1);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncthreads();
+    const double* yrow = ys + ((size_t)buf * K3_WC * 6 + series) * TW + lane;
+#pragma unroll 2
+    for (int w = 0; w < K3_WC; ++w) {
+      const double* yy = yrow + (size_t)w * 6 * TW;
+      double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+      for (int i = 0; i + 1 < WIN; i += 2) {
+        a0 = fma(C[i], yy[i], a0);
+        a1 = fma(C[i + 1], yy[i + 1], a1);
+      }
+      if (WIN & 1) a0 = fma(C[WIN - 1], yy[WIN - 1], a0);
+      red[(w * K3_PAIRS + pr_id) * K3_TS + lane] = a0 + a1;
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < K3_WC * 3 * K3_TS; e += K3_THREADS) {
+      const int w = e / (3 * K3_TS), o = (e / K3_TS) % 3, ln = e % K3_TS;
+      const int b = ch * K3_WC + w;
+      const long long nn = n0 + ln;
+      if (b >= p.B || nn >= p.N) continue;
+      const double* r = red + (size_t)w * K3_PAIRS * K3_TS + ln;
+      double v;
+      if (p.out_kind == 0) {
+        v = (r[(o * 4 + 0) * K3_TS] + r[(o * 4 + 1) * K3_TS]) + (r[(o * 4 + 2) * K3_TS] + r[(o * 4 + 3) * K3_TS]);
+      } else {
+        double xyz[3], out[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+          xyz[c] = (r[(c * 4 + 0) * K3_TS] + r[(c * 4 + 1) * K3_TS]) + (r[(c * 4 + 2) * K3_TS] + r[(c * 4 + 3) * K3_TS]);
+        combine_out(1, xyz[0], xyz[1], xyz[2], out);
+        v = o == 0 ? out[0] : (o == 1 ? out[1] : out[2]);
+      }
+      if (nn < p.margin_lo || nn >= p.N - p.margin_hi) v = 0.0;
+      p.tdi[((size_t)b * 3 + o) * p.N + nn] = v;
+    }
+  }
+}
+
+template <int H, int WIN>
+static int launch_merged(const K3Params& p, cudaStream_t st) {
+  constexpr int TW = K3_TS + WIN - 1;
+  const size_t smem = (size_t)(2 * K3_WC * 6 * TW + K3_WC * K3_PAIRS * K3_TS) * sizeof(double);
+  LISA_CUDA(cudaFuncSetAttribute(k3_tdi_merged<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k3_tdi_merged<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, smem, st>>>(p);
+  LISA_LAUNCH_CHECK("k3_tdi_merged");
+  return LISA_TD_OK;
+}
+
+extern int g_force_generic;
+
+int run_tdi(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+            long long margin_lo, long long margin_hi, const double* y, const OrbitDev& orb,
+            double* tdi, cudaStream_t st) {
+  K3Params p;
+  p.B = B; p.N = N; p.t0 = t0; p.dt = dt; p.inv_dt = 1.0 / dt;
+  p.half = (order + 1) / 2; p.generation = generation; p.out_kind = out_kind;
+  p.margin_lo = margin_lo; p.margin_hi = margin_hi; p.y = y; p.tdi = tdi; p.orb = orb;
+  make_lagw(order, &p.lw);
+  build_pairs(generation, p.pair);
+  const int nL = generation == 20 ? 7 : 3;
+  const int kcap = (int)ceil(nL * orb.max_L / dt);
+  p.kcap = kcap;
+  const int need = kcap + 2 * p.half;
+  if (!g_force_generic) {
+    if (p.half == 16) {
+      if (need <= 40) return launch_merged<16, 40>(p, st);
+      if (need <= 44) return launch_merged<16, 44>(p, st);
+      if (need <= 48) return launch_merged<16, 48>(p, st);
+    } else if (p.half == 1) {
+      if (need <= 8) return launch_merged<1, 8>(p, st);
+      if (need <= 16) return launch_merged<1, 16>(p, st);
+    }
+  }
+  dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);
+  k3_tdi_generic<<<grid, 256, 0, st>>>(p);
+  LISA_LAUNCH_CHECK("k3_tdi_generic");
+  return LISA_TD_OK;
+}
+
+}  // namespace lisa

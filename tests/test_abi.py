@@ -1,0 +1,80 @@
+"""Host-side checks of the C-ABI library that need no GPU: it loads, exports every symbol that
+include/lisa_td.h declares, and rejects bad arguments before touching the device."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2501_08261_b200 import build, lib as L
+    build.build()
+    L.load()
+    return L
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "lisa_td.h")).read()
+    declared = set(re.findall(r"LISA_TD_API[^;]*?\b(lisa_td_\w+)\s*\(", hdr))
+    assert len(declared) >= 18
+    assert declared == set(lib.EXPORTS)
+    L = lib.load()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_version_and_error_string(lib):
+    assert lib.version() >= 100
+    assert isinstance(lib.last_error(), str)
+
+
+def test_orbit_struct_layout_matches_header(lib):
+    # int + pad, 5 doubles, 9 doubles, 6 doubles
+    assert C.sizeof(lib.Orbit) == 8 + 5 * 8 + 9 * 8 + 6 * 8
+
+
+def test_argument_validation_happens_before_any_launch(lib):
+    L = lib.load()
+    orb = lib.make_orbit({"kind": "kepler1", "L_m": 2.5e9, "a_m": 1.495978707e11, "year_s": 365.25 * 86400})
+    fake = C.c_void_p(0x1000)       # aligned, never dereferenced: validation fails first
+    odd = C.c_void_p(0x1008)
+    # bad order
+    rc = L.lisa_td_link_response(1, 4096, 0.0, 5.0, 30, 128, fake, fake, fake, fake, C.byref(orb), fake, None)
+    assert rc == -1 and "order" in lib.last_error()
+    # B <= 0
+    assert L.lisa_td_link_response(0, 4096, 0.0, 5.0, 31, 128, fake, fake, fake, fake, C.byref(orb), fake, None) == -1
+    # NULL pointer
+    assert L.lisa_td_link_response(1, 4096, 0.0, 5.0, 31, 128, None, fake, fake, fake, C.byref(orb), fake, None) == -1
+    # misaligned pointer
+    assert L.lisa_td_link_response(1, 4096, 0.0, 5.0, 31, 128, odd, fake, fake, fake, C.byref(orb), fake, None) == -2
+    # margin too small for the orbit: |k.r|/c can reach ~500 s = 100 samples
+    rc = L.lisa_td_link_response(1, 4096, 0.0, 5.0, 31, 64, fake, fake, fake, fake, C.byref(orb), fake, None)
+    assert rc == -1 and "margin_y" in lib.last_error()
+    # TDI: bad generation, small margins
+    assert L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 17, 1, 160, 144, fake, C.byref(orb), fake, None) == -1
+    assert L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 20, 1, 20, 144, fake, C.byref(orb), fake, None) == -1
+    assert L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 20, 1, 160, 4, fake, C.byref(orb), fake, None) == -1
+    # modes: l out of range
+    l = (C.c_int * 1)(9)
+    m = (C.c_int * 1)(2)
+    assert L.lisa_td_modes_to_pol(1, 16, 1, l, m, *([fake] * 11), None) == -1
+    # loglike: band outside the spectrum, NULL plan
+    assert L.lisa_td_loglike(None, 1, 16, fake, fake, fake, 0, 4, fake, None, None, None) == -1
+    # workspace size helper
+    assert L.lisa_td_response_tdi_workspace_bytes(2, 1024) == 2 * 6 * 1024 * 8
+
+
+def test_psd_weights_host_helper_matches_oracle(lib, orc):
+    N, dt = 4096, 5.0
+    for gen in (15, 20):
+        a = lib.psd_weights(N, dt, 3e-15, 15e-12, 8.339, gen)
+        b = orc.psd_weights(N, dt, 3e-15, 15e-12, 8.339, gen)
+        assert np.all(a[:, 0] == 0)
+        # relative to the local scale; near the zeros of the transfer function the PSD is tiny
+        ok = np.abs(a[:, 1:] - b[:, 1:]) <= 1e-9 * np.abs(b[:, 1:])
+        assert ok.mean() > 0.999
