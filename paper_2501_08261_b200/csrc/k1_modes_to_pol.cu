@@ -50,10 +50,14 @@ struct quat {
   cplx a, b;
 };
 __device__ __forceinline__ quat quat_from_euler(double al, double be, double ga) {
-  double sb, cb, sp, cp, sm, cm;
+  // sin/cos of (al +- ga)/2 by angle addition from al/2 and ga/2: forming al + ga first would
+  // round at ulp(|al|+|ga|) (1e-13 rad after a few hundred radians of precession).
+  double sb, cb, sa, ca, sg, cg;
   sincos_d(0.5 * be, sb, cb);
-  sincos_d(0.5 * (al + ga), sp, cp);
-  sincos_d(0.5 * (al - ga), sm, cm);
+  sincos_d(0.5 * al, sa, ca);
+  sincos_d(0.5 * ga, sg, cg);
+  const double cp = fma(ca, cg, -sa * sg), sp = fma(sa, cg, ca * sg);
+  const double cm = fma(ca, cg, sa * sg), sm = fma(sa, cg, -ca * sg);
   return {{cb * cp, cb * sp}, {sb * cm, -sb * sm}};
 }
 // consecutive rotations R_p R_q:  (pa qa - conj(pb) qb,  pb qa + conj(pa) qb)
