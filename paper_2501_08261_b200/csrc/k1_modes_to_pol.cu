@@ -163,6 +163,96 @@ __global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol(const K1Params p) 
   }
 }
 
+// ---------------------------------------------------------------- five-mode fast path
+// For the paper's mode set {(2,2),(2,1),(3,3),(4,4),(5,5)} ("the 5-mode model")
+// and any subset of it, every frakD^l_{+-m,2} is a monomial in Qa, Qb and their conjugates.
+// With z = Qa conj(Qb):
+//   N2 D^2_{2,2} = N2 Qa^4          N2 D^2_{-2,2} = N2 Qb^4
+//   N2 D^2_{1,2} = 2 N2 Qa^3 Qb     N2 D^2_{-1,2} = 2 N2 Qa Qb^3
+//   Nl D^l_{l,2} = c_l Qa^4 z^{l-2} (-)^l Nl D^l_{-l,2} = c_l Qb^4 conj(z)^{l-2},  l = 3,4,5
+//   c3 = -sqrt(6) N3, c4 = 2 sqrt(7) N4, c5 = -sqrt(120) N5
+// so  H = Qa^4 G + Qb^4 conj(G) + 2 N2 Qa Qb (Qa^2 h21 + Qb^2 conj(h21)),
+//     G = N2 h22 + z (c3 h33 + z (c4 h44 + z c5 h55)).
+// Everything stays in registers (the generic kernel keeps power tables in local memory).
+struct K1FastParams {
+  int B;
+  long long N;
+  int n_modes, twisted, have_e0;
+  int idx[5];  // position of (2,2),(2,1),(3,3),(4,4),(5,5) in the mode list, -1 = absent
+  double c22, c21, c33, c44, c55;
+  const double *amp, *phase, *alpha, *beta, *gamma, *iota, *phi, *psi, *euler0;
+  double *hplus, *hcross;
+};
+
+struct K1Pre {
+  cplx Fa, Fb, z, qa2, qb2, qab;
+};
+__device__ __forceinline__ K1Pre k1_pre(const quat& q) {
+  K1Pre r;
+  r.qa2 = cmul(q.a, q.a);
+  r.qb2 = cmul(q.b, q.b);
+  r.Fa = cmul(r.qa2, r.qa2);
+  r.Fb = cmul(r.qb2, r.qb2);
+  r.z = cmul(q.a, cconj(q.b));
+  r.qab = cmul(q.a, q.b);
+  return r;
+}
+
+__global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol_std5(const K1FastParams p) {
+  __shared__ quat Qc;
+  __shared__ double rot[2];
+  const int b = blockIdx.y;
+  if (threadIdx.x == 0) {
+    quat q = quat_from_euler(p.phi[b], p.iota[b], 0.0);  // footnote 1
+    if (p.have_e0)
+      q = quat_mul(quat_from_euler(p.euler0[3 * b], p.euler0[3 * b + 1], p.euler0[3 * b + 2]), q);
+    Qc = q;
+    double s2, c2;
+    sincos_d(2.0 * p.psi[b], s2, c2);
+    rot[0] = c2;
+    rot[1] = s2;
+  }
+  __syncthreads();
+  const size_t bN = (size_t)b * p.N;
+  const double* amp = p.amp + bN * p.n_modes;
+  const double* pha = p.phase + bN * p.n_modes;
+  const quat qc = Qc;
+  K1Pre pre = k1_pre(qc);
+  const long long n_base = (long long)blockIdx.x * (K1_THREADS * K1_PER_THREAD);
+#pragma unroll 1
+  for (int it = 0; it < K1_PER_THREAD; ++it) {
+    const long long n = n_base + it * K1_THREADS + threadIdx.x;
+    if (n >= p.N) break;
+    if (p.twisted) pre = k1_pre(quat_mul(quat_from_euler(p.alpha[bN + n], p.beta[bN + n], p.gamma[bN + n]), qc));
+    // h_k = a (cos phi - i sin phi), scaled by its constant
+    cplx h[5];
+    const double cc[5] = {p.c22, p.c21, p.c33, p.c44, p.c55};
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      h[k] = {0.0, 0.0};
+      if (p.idx[k] >= 0) {
+        double s, c;
+        const double a = amp[(size_t)p.idx[k] * p.N + n] * cc[k];
+        sincos_d(pha[(size_t)p.idx[k] * p.N + n], s, c);
+        h[k] = {a * c, -a * s};
+      }
+    }
+    // G = h22 + z (h33 + z (h44 + z h55))
+    cplx g = cmul(pre.z, h[4]);
+    g = {g.re + h[3].re, g.im + h[3].im};
+    g = cmul(pre.z, g);
+    g = {g.re + h[2].re, g.im + h[2].im};
+    g = cmul(pre.z, g);
+    g = {g.re + h[0].re, g.im + h[0].im};
+    cplx t1 = cmul(pre.Fa, g), t2 = cmul(pre.Fb, cconj(g));
+    cplx u1 = cmul(pre.qa2, h[1]), u2 = cmul(pre.qb2, cconj(h[1]));
+    cplx u = cmul(pre.qab, {u1.re + u2.re, u1.im + u2.im});
+    const double Hre = (t1.re + t2.re) + u.re, Him = (t1.im + t2.im) + u.im;
+    p.hplus[bN + n] = fma(Hre, rot[0], -Him * rot[1]);
+    p.hcross[bN + n] = -fma(Hre, rot[1], Him * rot[0]);
+  }
+}
+
 static double factorial_ld(int n) {
   long double f = 1;
   for (int i = 2; i <= n; ++i) f *= i;
@@ -175,11 +265,42 @@ static long double binom_ld(int n, int k) {
   return r;
 }
 
+extern int g_force_generic;
+
 int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m, const double* amp,
                      const double* phase, const double* alpha, const double* beta,
                      const double* gamma, const double* iota, const double* phi,
                      const double* psi, const double* euler0, double* hplus, double* hcross,
                      cudaStream_t st) {
+  // fast path: the mode list is a subset of {(2,2),(2,1),(3,3),(4,4),(5,5)}, each at most once
+  {
+    static const int SL[5] = {2, 2, 3, 4, 5}, SM[5] = {2, 1, 3, 4, 5};
+    K1FastParams f;
+    bool ok = !g_force_generic;
+    for (int j = 0; j < 5; ++j) f.idx[j] = -1;
+    for (int k = 0; k < n_modes && ok; ++k) {
+      int j = 0;
+      while (j < 5 && !(SL[j] == l[k] && SM[j] == m[k])) ++j;
+      if (j == 5 || f.idx[j] >= 0) ok = false;
+      else f.idx[j] = k;
+    }
+    if (ok) {
+      const long double PI_L = 3.14159265358979323846264338327950288L;
+      auto NL = [&](int ll) { return sqrtl((2 * ll + 1) / (4 * PI_L)); };
+      f.c22 = (double)NL(2);
+      f.c21 = (double)(2 * NL(2));
+      f.c33 = (double)(-sqrtl(6.0L) * NL(3));
+      f.c44 = (double)(2 * sqrtl(7.0L) * NL(4));
+      f.c55 = (double)(-sqrtl(120.0L) * NL(5));
+      f.B = B; f.N = N; f.n_modes = n_modes; f.twisted = alpha != nullptr; f.have_e0 = euler0 != nullptr;
+      f.amp = amp; f.phase = phase; f.alpha = alpha; f.beta = beta; f.gamma = gamma;
+      f.iota = iota; f.phi = phi; f.psi = psi; f.euler0 = euler0; f.hplus = hplus; f.hcross = hcross;
+      dim3 grid((unsigned)((N + K1_THREADS * K1_PER_THREAD - 1) / (K1_THREADS * K1_PER_THREAD)), (unsigned)B);
+      k1_modes_to_pol_std5<<<grid, K1_THREADS, 0, st>>>(f);
+      LISA_LAUNCH_CHECK("k1_modes_to_pol_std5");
+      return LISA_TD_OK;
+    }
+  }
   K1Params p;
   p.B = B; p.N = N; p.n_modes = n_modes; p.twisted = alpha != nullptr; p.have_e0 = euler0 != nullptr;
   p.amp = amp; p.phase = phase; p.alpha = alpha; p.beta = beta; p.gamma = gamma;

@@ -44,7 +44,7 @@ __device__ __forceinline__ void read_pair(const double2* __restrict__ tile, int 
 }
 
 template <int HT>
-__global__ void __launch_bounds__(K2_THREADS) k2_link_response(const K2Params p) {
+__global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params p) {
   extern __shared__ double2 tile[];  // [TILE + 2*margin]
   __shared__ double sky[9];          // k, u, v of this walker (Eq. 2.7)
   const int b = blockIdx.y;

@@ -79,7 +79,11 @@ def _s1_inputs(rng, modes, B, N, big_phase=True):
 @pytest.mark.parametrize("modes", [[(2, 2)], MODES5, MODES_GEN])
 @pytest.mark.parametrize("twisted", [False, True])
 @pytest.mark.parametrize("with_e0", [False, True])
-def test_s1_parity(lib, orc, modes, twisted, with_e0):
+@pytest.mark.parametrize("force_generic", [False, True])
+def test_s1_parity(lib, orc, modes, twisted, with_e0, force_generic):
+    """force_generic=False takes the five-mode fast kernel for the first two mode lists."""
+    if force_generic and len(modes) > 5:
+        pytest.skip("already the generic kernel")
     rng = np.random.default_rng(11 + len(modes) + 2 * twisted + with_e0)
     B, N = 3, 2500  # several blocks and a ragged tail
     l, m = zip(*modes)
@@ -87,7 +91,11 @@ def test_s1_parity(lib, orc, modes, twisted, with_e0):
     ang = [rng.uniform(-400, 400, (B, N)), rng.uniform(0, math.pi, (B, N)), rng.uniform(-400, 400, (B, N))] if twisted else [None] * 3
     e0 = rng.uniform(0.1, 1.5, (B, 3)) if with_e0 else None
     ref = orc.modes_to_pol(l, m, amp, phase, iota, phi, psi, *ang, euler0=e0)
-    got = gpu_s1(lib, l, m, amp, phase, iota, phi, psi, *ang, euler0=e0)
+    lib.debug_force_generic(force_generic)
+    try:
+        got = gpu_s1(lib, l, m, amp, phase, iota, phi, psi, *ang, euler0=e0)
+    finally:
+        lib.debug_force_generic(False)
     scale = np.sum(amp, axis=1)
     for g, r in zip(got, ref):
         # up to l+2 = 10 chained complex products per row and 2 n_modes rows: a few 1e-16 each
