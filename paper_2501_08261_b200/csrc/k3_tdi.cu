@@ -149,11 +149,30 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
   for (int c = 0; c < 3; ++c) ob[(size_t)c * p.N + n] = o[c];
 }
 
-// ---------------------------------------------------------------- merged-stencil kernel
-constexpr int K3_TS = 32;       // output samples per block (one warp lane each)
-constexpr int K3_PAIRS = 12;    // warps per block: channel x series
-constexpr int K3_THREADS = K3_TS * K3_PAIRS;
-constexpr int K3_WC = 8;        // walkers per shared-memory chunk
+// ---------------------------------------------------------------- merged-stencil DMMA kernel
+// Block = K3_TS = 32 output samples x ALL walkers.
+//
+// Phase 1 (once per block): warp = (channel, series) pair, lane = sample.  Each thread merges
+// the 4 (generation 2) or 2 (generation 1.5) delayed reads of its pair into ONE stencil of WIN
+// taps (the interpolation is linear in y: sum_t s_t sum_j c_j(eps_t) y[n-K_t+j] = sum_i C_i
+// y[n+LOW+i]) and parks it in shared memory.  The light travel times of the 32 samples are
+// evaluated once (32 threads) and shared.
+//
+// Phase 2: the merged stencils form, per pair, a banded matrix Cband[n][m]; the output is the
+// banded product  out[n][w] = sum_pairs sum_m Cband_p[n][m] y_{series(p)}[m][w]  over the
+// walkers w -- the one dense-ish contraction on this path whose left operand does NOT depend
+// on the walker.  It runs on the FP64 tensor path (mma.sync m8n8k4 f64 -> DMMA.8x8x4): warp =
+// (channel, block of 8 samples), A fragments (4 pairs x KSTEPS) live in registers for the
+// whole block, B fragments (y of 8 walkers x 4 times) are one conflict-free LDS.64 each, and
+// the four pairs of a channel accumulate in the same two accumulator registers.  One LDS.64
+// per 8 FMA instead of one per FMA (the previous SIMT version was shared-memory bound at 22 %
+// FP64-pipe activity).  Walkers stream through shared memory in chunks of 16 (cp.async,
+// double buffered); X,Y,Z of a chunk meet in shared memory for the A,E,T combination.
+constexpr int K3_TS = 32;                  // output samples per block
+constexpr int K3_PAIRS = 12;               // (channel, series) pairs
+constexpr int K3_THREADS = 32 * K3_PAIRS;  // 12 warps
+constexpr int K3_WC = 16;                  // walkers per shared-memory chunk (two MMA N-blocks)
+constexpr int K3_XS = K3_WC + 1;           // row stride of the X,Y,Z exchange buffer
 
 __device__ __forceinline__ void cp_async8_zfill(void* smem, const void* gmem, bool valid) {
   unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -164,6 +183,13 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int NKEEP>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP));
+}
+// D(8x8) += A(8x4, row) * B(4x8, col), fp64.  Lane l holds A[l/4][l%4], B[l%4][l/4] and
+// D[l/4][2(l%4) + {0,1}].
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
 }
 
 // Adds sgn * c_j(eps) into the merged stencil at compile-time offset OFF.
@@ -196,42 +222,89 @@ struct TermDispatch<H, WIN, -1> {
 };
 
 template <int H, int WIN>
-__global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_merged(const K3Params p) {
-  constexpr int KCAP = WIN - 2 * H;       // largest integer delay the window can hold
-  constexpr int TW = K3_TS + WIN - 1;     // y samples per row of the tile
-  constexpr int LOW = -(KCAP + H - 1);    // offset of stencil tap 0 relative to n
-  extern __shared__ double smem[];
-  double* ys = smem;                                   // [2][WC][6][TW]
-  double* red = smem + 2 * K3_WC * 6 * TW;             // [WC][12][32]
-  const int lane = threadIdx.x & 31;
-  const int pr_id = threadIdx.x >> 5;
-  const long long n0 = (long long)blockIdx.x * K3_TS;
-  const long long n = n0 + lane;
+struct K3Geom {
+  static constexpr int KCAP = WIN - 2 * H;            // largest integer delay the window holds
+  static constexpr int LOW = -(KCAP + H - 1);         // offset of stencil tap 0 relative to n
+  static constexpr int KSTEPS = (WIN + 7 + 3) / 4;    // k-steps of one 8-sample row block
+  static constexpr int TWMIN = 24 + 4 * KSTEPS;       // y samples a block touches per series
+  static constexpr int TW = TWMIN + ((2 - TWMIN % 4) + 4) % 4;  // == 2 mod 4: walker stride 6 TW == 4 or 12 mod 16
+  static constexpr int CS = ((WIN + 2) / 8) * 8 + 5;  // odd, >= WIN, (CS-1) == 4 mod 8: conflict-free fragment reads
+  static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
+  static constexpr int CBUF = K3_PAIRS * K3_TS * CS;  // doubles of the stencil staging area
+  static constexpr int XBUF = 3 * K3_TS * K3_XS;
+  static constexpr int UNION = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
+  static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
+};
 
-  // ---- phase 1: merged stencil of my (channel, series) pair at my sample, in registers
-  double C[WIN];
-#pragma unroll
-  for (int i = 0; i < WIN; ++i) C[i] = 0.0;
-  const K3Pair& pr = p.pair[pr_id];
-  if (n >= p.margin_lo && n < p.N - p.margin_hi) {
+template <int H, int WIN>
+__global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
+  using G = K3Geom<H, WIN>;
+  constexpr int KCAP = G::KCAP, LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, CS = G::CS;
+  static_assert(CS >= WIN && (CS & 1), "stencil row stride");
+  extern __shared__ double smem[];
+  double* ys = smem;                    // [2][WC][6][TW]   (phase 2)
+  double* cbuf = smem;                  // [12][32][CS]     (phase 1, aliased)
+  double* xs = smem + G::UNION;         // [3][32][XS]
+  double* Ls = xs + G::XBUF;            // [32][6]
+  const int lane = threadIdx.x & 31;
+  const int wid = threadIdx.x >> 5;
+  const long long n0 = (long long)blockIdx.x * K3_TS;
+
+  // ---- phase 1a: light travel times of the 32 samples
+  if (wid == 0) {
     double L[6];
-    orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
-    for (int k = 0; k < pr.n_terms; ++k) {
-      const double D = term_delay(pr.t[k], L, p.inv_dt);
-      const double Kf = ceil(D);
-      const double eps = Kf - D;
-      int off = KCAP - (int)Kf;
-      off = max(0, min(off, KCAP));
-      TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.lw);
+    orbit_arm_times(p.orb, fma((double)(n0 + lane), p.dt, p.t0), L);
+#pragma unroll
+    for (int l = 0; l < 6; ++l) Ls[lane * 6 + l] = L[l];
+  }
+  __syncthreads();
+  // ---- phase 1b: merged stencil of (pair = wid, sample = lane)
+  {
+    double C[WIN];
+#pragma unroll
+    for (int i = 0; i < WIN; ++i) C[i] = 0.0;
+    const K3Pair& pr = p.pair[wid];
+    const long long n = n0 + lane;
+    if (n >= p.margin_lo && n < p.N - p.margin_hi) {
+      double L[6];
+#pragma unroll
+      for (int l = 0; l < 6; ++l) L[l] = Ls[lane * 6 + l];
+      for (int k = 0; k < pr.n_terms; ++k) {
+        const double D = term_delay(pr.t[k], L, p.inv_dt);
+        const double Kf = ceil(D);
+        const double eps = Kf - D;
+        int off = KCAP - (int)Kf;
+        off = max(0, min(off, KCAP));
+        TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.lw);
+      }
+    }
+    double* dst = cbuf + (size_t)(wid * K3_TS + lane) * CS;
+#pragma unroll
+    for (int i = 0; i < WIN; ++i) dst[i] = C[i];
+  }
+  __syncthreads();
+  // ---- phase 1c: A fragments of (channel ch, row block rb): 4 pairs x KSTEPS values
+  const int ch = wid >> 2, rb = wid & 3;
+  const int r = lane >> 2, kk = lane & 3;
+  double A[4][KSTEPS];
+  int ser[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    ser[q] = p.pair[ch * 4 + q].series;
+    const double* src = cbuf + (size_t)((ch * 4 + q) * K3_TS + rb * 8 + r) * CS;
+#pragma unroll
+    for (int ks = 0; ks < KSTEPS; ++ks) {
+      const int i = 4 * ks + kk - r;
+      A[q][ks] = (i >= 0 && i < WIN) ? src[i] : 0.0;
     }
   }
-  const int series = pr.series;
+  __syncthreads();  // cbuf is dead from here on: its space becomes the y buffers
 
   // ---- phase 2: stream walkers
   const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
   auto prefetch = [&](int chunk, int buf) {
-    double* dst = ys + (size_t)buf * K3_WC * 6 * TW;
-    for (int e = threadIdx.x; e < K3_WC * 6 * TW; e += K3_THREADS) {
+    double* dst = ys + (size_t)buf * G::YBUF;
+    for (int e = threadIdx.x; e < G::YBUF; e += K3_THREADS) {
       const int row = e / TW, i = e - row * TW;
       const int w = chunk * K3_WC + row / 6;
       const long long g = n0 + LOW + i;
@@ -242,46 +315,44 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_merged(const K3Params p)
     cp_async_commit();
   };
   prefetch(0, 0);
-  for (int ch = 0; ch < n_chunks; ++ch) {
-    const int buf = ch & 1;
-    if (ch + 1 < n_chunks) {
-      prefetch(ch + 1, buf ^ 1);
+  for (int c = 0; c < n_chunks; ++c) {
+    const int buf = c & 1;
+    if (c + 1 < n_chunks) {
+      prefetch(c + 1, buf ^ 1);
       cp_async_wait<1>();
     } else {
       cp_async_wait<0>();
     }
-    __syncthreads();
-    const double* yrow = ys + ((size_t)buf * K3_WC * 6 + series) * TW + lane;
-#pragma unroll 2
-    for (int w = 0; w < K3_WC; ++w) {
-      const double* yy = yrow + (size_t)w * 6 * TW;
-      double a0 = 0.0, a1 = 0.0;
+    __syncthreads();  // chunk c landed; everyone is done with xs of chunk c-1
+    // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
+    const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk;
+    double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
 #pragma unroll
-      for (int i = 0; i + 1 < WIN; i += 2) {
-        a0 = fma(C[i], yy[i], a0);
-        a1 = fma(C[i + 1], yy[i + 1], a1);
+    for (int q = 0; q < 4; ++q) {
+      const double* y0 = yb + ser[q] * TW;
+      const double* y1 = y0 + 8 * 6 * TW;
+#pragma unroll
+      for (int ks = 0; ks < KSTEPS; ++ks) {
+        dmma884(d00, d01, A[q][ks], y0[4 * ks]);
+        dmma884(d10, d11, A[q][ks], y1[4 * ks]);
       }
-      if (WIN & 1) a0 = fma(C[WIN - 1], yy[WIN - 1], a0);
-      red[(w * K3_PAIRS + pr_id) * K3_TS + lane] = a0 + a1;
+    }
+    {
+      double* xr = xs + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
+      xr[0] = d00; xr[1] = d01; xr[8] = d10; xr[9] = d11;
     }
     __syncthreads();
     for (int e = threadIdx.x; e < K3_WC * 3 * K3_TS; e += K3_THREADS) {
-      const int w = e / (3 * K3_TS), o = (e / K3_TS) % 3, ln = e % K3_TS;
-      const int b = ch * K3_WC + w;
+      const int ln = e & 31, o = (e >> 5) % 3, w = e / 96;
+      const int b = c * K3_WC + w;
       const long long nn = n0 + ln;
       if (b >= p.B || nn >= p.N) continue;
-      const double* r = red + (size_t)w * K3_PAIRS * K3_TS + ln;
-      double v;
-      if (p.out_kind == 0) {
-        v = (r[(o * 4 + 0) * K3_TS] + r[(o * 4 + 1) * K3_TS]) + (r[(o * 4 + 2) * K3_TS] + r[(o * 4 + 3) * K3_TS]);
-      } else {
-        double xyz[3], out[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-          xyz[c] = (r[(c * 4 + 0) * K3_TS] + r[(c * 4 + 1) * K3_TS]) + (r[(c * 4 + 2) * K3_TS] + r[(c * 4 + 3) * K3_TS]);
-        combine_out(1, xyz[0], xyz[1], xyz[2], out);
-        v = o == 0 ? out[0] : (o == 1 ? out[1] : out[2]);
-      }
+      const double X = xs[(0 * K3_TS + ln) * K3_XS + w];
+      const double Y = xs[(1 * K3_TS + ln) * K3_XS + w];
+      const double Z = xs[(2 * K3_TS + ln) * K3_XS + w];
+      double out[3];
+      combine_out(p.out_kind, X, Y, Z, out);
+      double v = o == 0 ? out[0] : (o == 1 ? out[1] : out[2]);
       if (nn < p.margin_lo || nn >= p.N - p.margin_hi) v = 0.0;
       p.tdi[((size_t)b * 3 + o) * p.N + nn] = v;
     }
@@ -289,12 +360,12 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_merged(const K3Params p)
 }
 
 template <int H, int WIN>
-static int launch_merged(const K3Params& p, cudaStream_t st) {
-  constexpr int TW = K3_TS + WIN - 1;
-  const size_t smem = (size_t)(2 * K3_WC * 6 * TW + K3_WC * K3_PAIRS * K3_TS) * sizeof(double);
-  LISA_CUDA(cudaFuncSetAttribute(k3_tdi_merged<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k3_tdi_merged<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, smem, st>>>(p);
-  LISA_LAUNCH_CHECK("k3_tdi_merged");
+static int launch_mma(const K3Params& p, cudaStream_t st) {
+  using G = K3Geom<H, WIN>;
+  static_assert(G::SMEM <= 227 * 1024, "k3_tdi_mma shared memory");
+  LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+  k3_tdi_mma<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, G::SMEM, st>>>(p);
+  LISA_LAUNCH_CHECK("k3_tdi_mma");
   return LISA_TD_OK;
 }
 
@@ -315,12 +386,12 @@ int run_tdi(int B, long long N, double t0, double dt, int order, int generation,
   const int need = kcap + 2 * p.half;
   if (!g_force_generic) {
     if (p.half == 16) {
-      if (need <= 40) return launch_merged<16, 40>(p, st);
-      if (need <= 44) return launch_merged<16, 44>(p, st);
-      if (need <= 48) return launch_merged<16, 48>(p, st);
+      if (need <= 40) return launch_mma<16, 40>(p, st);
+      if (need <= 44) return launch_mma<16, 44>(p, st);
+      if (need <= 48) return launch_mma<16, 48>(p, st);
     } else if (p.half == 1) {
-      if (need <= 8) return launch_merged<1, 8>(p, st);
-      if (need <= 16) return launch_merged<1, 16>(p, st);
+      if (need <= 8) return launch_mma<1, 8>(p, st);
+      if (need <= 16) return launch_mma<1, 16>(p, st);
     }
   }
   dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);
