@@ -43,6 +43,37 @@ void make_lagw(int order, LagW* out) {
   }
 }
 
+void make_lags(int order, LagS* out) {
+  const int H = (order + 1) / 2;
+  long double w[MAX_HALF];
+  long double logabs = 0.0L;
+  int neg = 0;
+  for (int k = 1; k <= H; ++k) {
+    long double f = 1.0L;  // (k+H-1)! (H-k)!
+    for (int i = 2; i <= k + H - 1; ++i) f *= i;
+    for (int i = 2; i <= H - k; ++i) f *= i;
+    w[k - 1] = 1.0L / f;
+    if ((H - k) & 1) {
+      w[k - 1] = -w[k - 1];
+      ++neg;
+    }
+    logabs += logl(fabsl(w[k - 1]));
+  }
+  const long double R = expl(logabs / H);  // |prod w|^(1/H)
+  for (int i = 0; i < MAX_HALF; ++i) out->rho[i] = out->rc[i] = 0.0;
+  // g is formed from the ROUNDED rho_k: g prod_{i != k} rho_i = R / rho_k (1 + O(1e-19)), so
+  // the effective weight of pair k is off from w_k by the rounding of rho_k alone (<= 1.1e-16).
+  long double g = R;
+  for (int k = 1; k <= H; ++k) {
+    const double rho = (double)(R / w[k - 1]);
+    out->rho[k - 1] = rho;
+    out->rc[k - 1] = (double)((long double)rho * (long double)(k * (1 - k)));
+    g /= (long double)rho;
+  }
+  out->g = (double)g;
+  (void)neg;
+}
+
 // KEPLER1 on the host (long double), used only to bound |r| and L for margin validation.
 static void kepler1_host(const lisa_td_orbit* o, long double t, long double r[3][3]) {
   const long double PI_L = 3.14159265358979323846264338327950288L;

@@ -39,6 +39,19 @@ struct LagW {
 };
 void make_lagw(int order, LagW* out);
 
+// Scaled form of the same weights for the compile-time-order kernels.  With rho_k = R / w_k
+// and g = (prod_i w_i) / R^(H-1) one has  g * prod_{i != k} rho_i = w_k,  so the pair factors
+// can carry the weights:  Q'_k = rho_k (q + k(1-k)) = fma(rho[k-1], q, rc[k-1]),
+//   a_k = w_k prod_{i != k} Q_i = (g prod_{i<k} Q'_i) (prod_{i>k} Q'_i)
+// -- one FMA and three multiplies per node pair instead of an add and four multiplies.
+// R = |prod w_i|^(1/H) keeps every partial product far from over/underflow.
+struct LagS {
+  double rho[MAX_HALF];
+  double rc[MAX_HALF];
+  double g;
+};
+void make_lags(int order, LagS* out);
+
 // ------------------------------------------------------------------ orbit (device form)
 // KEPLER1 is evaluated as  r_k(t) = a (cos M, sin M, 0) + delta_k(t)  with the common 1 AU
 // part split off ALGEBRAICALLY (exact rearrangement of reading A8), so that arm vectors and
@@ -209,6 +222,63 @@ __device__ __forceinline__ void lagrange_dot2(double eps, int Hrt, const LagW& l
   }
   sp = ap + bp;
   sc = ac + bc;
+}
+
+// Compile-time half-width H, scaled weights (LagS): coefficient sweep + two dot products in
+// 7 + 4 fp64 ops per node pair.  c_k = a_k (eps + k - 1) = fma(a_k, k-1, a_k eps),
+// c_{1-k} = a_k (k - eps) = fma(a_k, k, -a_k eps).
+template <int H>
+__device__ __forceinline__ void lagrange_dot2s(double eps, const LagS& ls,
+                                               const double2* __restrict__ x, double& sp,
+                                               double& sc) {
+  double P[H + 1];
+  const double q = eps * (eps - 1.0);
+  P[1] = ls.g;
+#pragma unroll
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * fma(ls.rho[k - 1], q, ls.rc[k - 1]);
+  double S = 1.0, ap = 0.0, ac = 0.0, bp = 0.0, bc = 0.0;
+#pragma unroll
+  for (int k = H; k >= 1; --k) {
+    const double a = P[k] * S;
+    const double t = a * eps;
+    const double ck = fma(a, (double)(k - 1), t);
+    const double cm = fma(a, (double)k, -t);
+    const double2 xk = x[k], xm = x[1 - k];
+    ap = fma(ck, xk.x, ap);
+    ac = fma(ck, xk.y, ac);
+    bp = fma(cm, xm.x, bp);
+    bc = fma(cm, xm.y, bc);
+    if (k > 1) S *= fma(ls.rho[k - 1], q, ls.rc[k - 1]);
+  }
+  sp = ap + bp;
+  sc = ac + bc;
+}
+
+// Array-free ("Horner in node pairs") form of the same sum.  With S_k = prod_{i>k} Q'_i,
+//   sum_k P_k S_k v_k,  v_k = (eps+k-1) x_k + (k-eps) x_{1-k},
+// is the end value of  T_k = Q'_k T_{k-1} + P_k v_k,  T_0 = 0:  no prefix array, no suffix
+// chain, 11 fp64 ops per node pair for two series, and so few live registers that the tap
+// loads can be issued far ahead of their use.  HT > 0: unrolled; HT = 0: runtime half-width.
+template <int HT>
+__device__ __forceinline__ void lagrange_dot2h(double eps, int Hrt, const LagS& ls,
+                                               const double2* __restrict__ x, double& sp,
+                                               double& sc) {
+  const int H = HT > 0 ? HT : Hrt;
+  const double q = eps * (eps - 1.0);
+  double P = ls.g, Tp = 0.0, Tc = 0.0;
+#pragma unroll
+  for (int k = 1; k <= H; ++k) {
+    const double Q = fma(ls.rho[k - 1], q, ls.rc[k - 1]);
+    const double t = P * eps;
+    const double ck = k == 1 ? t : fma(P, (double)(k - 1), t);
+    const double cm = fma(P, (double)k, -t);
+    const double2 xk = x[k], xm = x[1 - k];
+    Tp = fma(Tp, Q, fma(ck, xk.x, cm * xm.x));
+    Tc = fma(Tc, Q, fma(ck, xk.y, cm * xm.y));
+    P *= Q;
+  }
+  sp = Tp;
+  sc = Tc;
 }
 
 // Same for a single series.

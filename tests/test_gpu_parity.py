@@ -158,7 +158,7 @@ def test_s2_generic_kernel_matches_specialised(lib, orc):
         b = gpu_s2(lib, hp, hc, lam, bet, orbit, 0.0, dt, 31, margin)
     finally:
         lib.debug_force_generic(False)
-    assert rel_l2(a, b) < 1e-15
+    assert rel_l2(a, b) < 1e-14  # two roundings of the same coefficients
 
 
 # ------------------------------------------------------------------------------------ S3
