@@ -112,6 +112,7 @@ int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
       mL = fmax(mL, o->L_static[l]);
     }
     d->max_r_over_c = mr / C_LIGHT;
+    d->max_off_over_c = mr / C_LIGHT;
     d->max_L = mL;
     return LISA_TD_OK;
   }
@@ -139,11 +140,15 @@ int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
     d->sn[k] = (double)sinl(2 * PI_L * k / 3);
   }
   // bounds over one orbital period (the motion is periodic), 4096 points, 0.1 % head-room
-  long double mr = 0, mL = 0;
+  long double mr = 0, mL = 0, mo = 0;
   for (int i = 0; i < 4096; ++i) {
     long double r[3][3];
-    kepler1_host(o, o->t_ref + (long double)o->year_s * i / 4096, r);
+    const long double ti = o->t_ref + (long double)o->year_s * i / 4096;
+    kepler1_host(o, ti, r);
+    const long double Mc = 2 * PI_L * (ti - o->t_ref) / o->year_s - o->phase0;
     for (int k = 0; k < 3; ++k) {
+      const long double ox = r[k][0] - a * cosl(Mc), oy = r[k][1] - a * sinl(Mc);
+      mo = fmaxl(mo, sqrtl(ox * ox + oy * oy + r[k][2] * r[k][2]));
       mr = fmaxl(mr, sqrtl(r[k][0] * r[k][0] + r[k][1] * r[k][1] + r[k][2] * r[k][2]));
       const int k2 = (k + 1) % 3;
       long double dx = r[k][0] - r[k2][0], dy = r[k][1] - r[k2][1], dz = r[k][2] - r[k2][2];
@@ -152,6 +157,7 @@ int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
   }
   d->max_r_over_c = (double)(mr * 1.001L / C_LIGHT);
   d->max_L = (double)(mL * 1.001L / C_LIGHT);
+  d->max_off_over_c = (double)(mo * 1.001L / C_LIGHT);
   return LISA_TD_OK;
 }
 

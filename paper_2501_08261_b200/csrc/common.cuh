@@ -67,6 +67,7 @@ struct OrbitDev {
   double L[6];                    // STATIC light travel times [s]
   double max_r_over_c;            // host-side bounds used for margin validation [s]
   double max_L;                   // [s]
+  double max_off_over_c;          // max |r_k - a(cos M, sin M, 0)| / c (STATIC: max |r_k| / c) [s]
 };
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* out);
 
@@ -273,6 +274,78 @@ __device__ __forceinline__ void lagrange_dot2h(double eps, int Hrt, const LagS& 
     const double ck = k == 1 ? t : fma(P, (double)(k - 1), t);
     const double cm = fma(P, (double)k, -t);
     const double2 xk = x[k], xm = x[1 - k];
+    Tp = fma(Tp, Q, fma(ck, xk.x, cm * xm.x));
+    Tc = fma(Tc, Q, fma(ck, xk.y, cm * xm.y));
+    P *= Q;
+  }
+  sp = Tp;
+  sc = Tc;
+}
+
+// Two ADJACENT output samples a, b = a+1 with the same integer delay: their windows are
+// x[e+1-H .. e+H] and x[e+2-H .. e+H+1], so one pass loads 2H+1 taps for both instead of 4H.
+// The series is stored split by parity of the element index (xe[i] = x[2i], xo[i] = x[2i+1])
+// so that a warp whose lanes own sample pairs (stride 2 elements) reads consecutive 16-byte
+// words -- conflict-free LDS.128.  e = element index of tap j = 0 of sample a.
+template <int HT>
+__device__ __forceinline__ void lagrange_dot2h_x2(double epsa, double epsb, int Hrt, const LagS& ls,
+                                                  const double2* __restrict__ xe,
+                                                  const double2* __restrict__ xo, int e,
+                                                  double (&sp)[2], double (&sc)[2]) {
+  const int H = HT > 0 ? HT : Hrt;
+  // x[e + o] = (o even ? p0[o/2] : p1[(o-1)/2])
+  const double2* p0 = ((e & 1) ? xo : xe) + (e >> 1);
+  const double2* p1 = (e & 1) ? xe + (e >> 1) + 1 : xo + (e >> 1);
+#define LISA_X(o) (((o) & 1) ? p1[((o) - 1) >> 1] : p0[(o) >> 1])
+  const double qa = epsa * (epsa - 1.0), qb = epsb * (epsb - 1.0);
+  double Pa = ls.g, Pb = ls.g, Tpa = 0.0, Tca = 0.0, Tpb = 0.0, Tcb = 0.0;
+  double2 ucur = LISA_X(1), dprev = ucur;  // x[e+k], x[e+2-k] at k = 1
+#pragma unroll
+  for (int k = 1; k <= H; ++k) {
+    const double2 unext = LISA_X(k + 1), dcur = LISA_X(1 - k);
+    const double rho = ls.rho[k - 1], rc = ls.rc[k - 1];
+    {  // sample a: taps x[e+k], x[e+1-k]
+      const double Q = fma(rho, qa, rc);
+      const double t = Pa * epsa;
+      const double ck = k == 1 ? t : fma(Pa, (double)(k - 1), t);
+      const double cm = fma(Pa, (double)k, -t);
+      Tpa = fma(Tpa, Q, fma(ck, ucur.x, cm * dcur.x));
+      Tca = fma(Tca, Q, fma(ck, ucur.y, cm * dcur.y));
+      Pa *= Q;
+    }
+    {  // sample b: taps x[e+1+k], x[e+2-k]
+      const double Q = fma(rho, qb, rc);
+      const double t = Pb * epsb;
+      const double ck = k == 1 ? t : fma(Pb, (double)(k - 1), t);
+      const double cm = fma(Pb, (double)k, -t);
+      Tpb = fma(Tpb, Q, fma(ck, unext.x, cm * dprev.x));
+      Tcb = fma(Tcb, Q, fma(ck, unext.y, cm * dprev.y));
+      Pb *= Q;
+    }
+    ucur = unext;
+    dprev = dcur;
+  }
+#undef LISA_X
+  sp[0] = Tpa; sc[0] = Tca; sp[1] = Tpb; sc[1] = Tcb;
+}
+
+// One sample from the parity-split storage (any element index): the rare path of a sample
+// pair whose integer delays differ.  Runtime loop, never unrolled (it is cold code).
+__device__ __forceinline__ void lagrange_dot2h_split(double eps, int H, const LagS& ls,
+                                                  const double2* __restrict__ xe,
+                                                  const double2* __restrict__ xo, int e,
+                                                  double& sp, double& sc) {
+  const double q = eps * (eps - 1.0);
+  double P = ls.g, Tp = 0.0, Tc = 0.0;
+#pragma unroll 1
+  for (int k = 1; k <= H; ++k) {
+    const int iu = e + k, id = e + 1 - k;
+    const double2 xk = (iu & 1) ? xo[iu >> 1] : xe[iu >> 1];
+    const double2 xm = (id & 1) ? xo[id >> 1] : xe[id >> 1];
+    const double Q = fma(ls.rho[k - 1], q, ls.rc[k - 1]);
+    const double t = P * eps;
+    const double ck = fma(P, (double)(k - 1), t);
+    const double cm = fma(P, (double)k, -t);
     Tp = fma(Tp, Q, fma(ck, xk.x, cm * xm.x));
     Tc = fma(Tc, Q, fma(ck, xk.y, cm * xm.y));
     P *= Q;

@@ -1,37 +1,44 @@
 // k2_link_response.cu -- S2: h+, hx -> six link responses (Eq. 2.7-2.8, PAPER.md:138-161;
 // readings A7, A8, A11 of DESIGN.md), and the link-level laser-noise helper (A12).
 //
-// One block = K2_T consecutive output samples (one per thread) x a group of up to K2_G walkers.
-// The orbit geometry of a sample -- spacecraft offsets, arm unit vectors, light travel times --
-// does not depend on the walker: each thread evaluates it ONCE and keeps it in registers
-// while the block loops over its walkers.  Per walker the strain tile with its halo
-// (+- margin_y samples) is staged in shared memory by cp.async (double buffered), interleaved
-// as (h+, hx) pairs so every stencil tap is one 16-byte LDS; the thread then forms the nine
-// distinct evaluation times (3 receivers + 6 emitters) and, for each, one fused "Lagrange
-// coefficient sweep + two dot products" (common.cuh).
+// One block = K2_T consecutive output samples x a group of up to K2_G walkers; a thread owns
+// TWO ADJACENT samples.
+//  - The orbit geometry of a sample (spacecraft offsets, arm lengths) does not depend on the
+//    walker: it is evaluated once per block into shared memory (geo[field][sample]) and reused
+//    by every walker of the group.
+//  - Per walker the strain tile is staged in shared memory by cp.async (double buffered) as
+//    (h+, hx) pairs, split by parity of the sample index (see lagrange_dot2h_x2).  The tile
+//    follows the walker's own 1 AU delay: it starts at n0 - Kc - halo with Kc = rint(Dc(n0)),
+//    so its length is K2_T + 2 halo (halo ~ 25 samples) whatever margin_y is.
+//  - Per sample pair: nine evaluation times (3 receivers + 6 emitters), each one fused
+//    "Lagrange coefficient sweep + two dot products" for both samples of the pair, which
+//    share all but one of their taps: 2H+1 shared-memory loads instead of 4H (the one-sample-
+//    per-thread version saturated the shared-memory pipe at 98 %, profiles/r1_s3_*.md).
 #include "common.cuh"
 
 namespace lisa {
+
+constexpr int K2_T = 512;        // output samples per block
+constexpr int K2_THREADS = 256;  // two adjacent samples per thread
+constexpr int K2_G = 16;         // walkers per block (upper bound)
+constexpr int K2_NGEO = 20;      // geometry fields per sample
 
 struct K2Params {
   int B;
   long long N;
   double t0, dt, inv_dt;
-  int half;  // (p+1)/2
-  int margin;
-  int group;  // walkers per block
+  int half;    // (p+1)/2
+  int margin;  // margin_y
+  int group;   // walkers per block
+  int halo;    // tile halo in samples (bound on |D - Kc| + half + slack)
   const double* hplus;
   const double* hcross;
   const double* lambda;
   const double* beta_sky;
   double* y;
   OrbitDev orb;
-  LagW lw;   // generic (runtime order) path
-  LagS ls;   // compile-time-order path
+  LagS ls;
 };
-
-constexpr int K2_T = 256;  // output samples per block = threads per block
-constexpr int K2_G = 16;   // walkers per block (upper bound)
 
 __device__ __forceinline__ void k2_cp_async8_zfill(void* smem, const void* gmem, bool valid) {
   unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -39,45 +46,41 @@ __device__ __forceinline__ void k2_cp_async8_zfill(void* smem, const void* gmem,
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(sa), "l"(gmem), "r"(sz));
 }
 
-// One fractional-delay read of (h+, hx) at delay D = Dc + Dl (samples).  The integer part is
-// decided from the rounded sum, the fraction is formed as (K - Dc) - Dl so that the common
-// 1 AU part (up to ~100 samples) does not cost the differential delays their low bits.
+// Fractional-delay reads of (h+, hx) for the sample pair (a, b = a+1) at delays
+// D = Dc + Dl (samples).  The integer part is decided from the rounded sum, the fraction is
+// formed as (K - Dc) - Dl so that the common 1 AU part (up to ~100 samples) does not cost the
+// differential delays their low bits.  ea0 = tile element of sample a at zero delay + Kc.
 template <int HT>
-__device__ __forceinline__ void read_pair(const double2* __restrict__ tile, int tile_len,
-                                          int n_rel, double Dc, double Dl, const K2Params& p,
-                                          double& vp, double& vc) {
-  const double Kf = ceil(Dc + Dl);
-  const double eps = (Kf - Dc) - Dl;
-  int b = n_rel - (int)Kf;  // tile index of tap j = 0
-  // memory safety only (validated margins keep the window inside the tile)
-  b = max(p.half - 1, min(b, tile_len - 1 - p.half));
-  lagrange_dot2h<HT>(eps, p.half, p.ls, tile + b, vp, vc);
+__device__ __forceinline__ void read_pair2(const double2* __restrict__ xe, const double2* __restrict__ xo,
+                                           int elo, int ehi, int ea0, const double (&Dc)[2],
+                                           double Dla, double Dlb, const K2Params& p,
+                                           double (&vp)[2], double (&vc)[2]) {
+  const double Ka = ceil(Dc[0] + Dla), Kb = ceil(Dc[1] + Dlb);
+  const double epsa = (Ka - Dc[0]) - Dla, epsb = (Kb - Dc[1]) - Dlb;
+  // memory safety only (the halo bound keeps every window inside the tile)
+  const int ea = max(elo, min(ea0 - (int)Ka, ehi));
+  if (Ka == Kb) {
+    lagrange_dot2h_x2<HT>(epsa, epsb, p.half, p.ls, xe, xo, ea, vp, vc);
+  } else {
+    const int eb = max(elo, min(ea0 + 1 - (int)Kb, ehi));
+    lagrange_dot2h_split(epsa, p.half, p.ls, xe, xo, ea, vp[0], vc[0]);
+    lagrange_dot2h_split(epsb, p.half, p.ls, xe, xo, eb, vp[1], vc[1]);
+  }
 }
 
 template <int HT, int KIND>
-__global__ void __launch_bounds__(K2_T, 3) k2_link_response(const K2Params p) {
-  extern __shared__ double2 tiles[];   // [2][K2_T + 2*margin] strain tiles, then geo[26][K2_T]
-  __shared__ double sky[K2_G][9];      // k, u, v of the block's walkers (Eq. 2.7)
+__global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params p) {
+  extern __shared__ double2 smem2[];  // [2 buffers][even, odd][LE] strain tiles, then geo[K2_NGEO][K2_T]
+  __shared__ double sky[K2_G][9];     // k, u, v of the block's walkers (Eq. 2.7)
+  __shared__ int Kc[K2_G];            // rint of the common 1 AU delay at the block's first sample
   const int R = p.margin;
-  const int tile_len = K2_T + 2 * R;
+  const int tile_len = K2_T + 2 * p.halo;
+  const int LE = (tile_len + 1) / 2 + 1;
   const long long n0 = (long long)blockIdx.x * K2_T;
   const int w0 = blockIdx.y * p.group;
   const int nw = min(p.group, p.B - w0);
-
-  auto prefetch = [&](int w, int buf) {
-    const double* hp = p.hplus + (size_t)(w0 + w) * p.N;
-    const double* hc = p.hcross + (size_t)(w0 + w) * p.N;
-    double2* dst = tiles + (size_t)buf * tile_len;
-    for (int i = threadIdx.x; i < tile_len; i += K2_T) {
-      const long long g = n0 - R + i;
-      const bool ok = g >= 0 && g < p.N;
-      const long long src = ok ? g : 0;
-      k2_cp_async8_zfill(&dst[i].x, hp + src, ok);
-      k2_cp_async8_zfill(&dst[i].y, hc + src, ok);
-    }
-    asm volatile("cp.async.commit_group;\n" ::);
-  };
-  prefetch(0, 0);
+  double* geo = reinterpret_cast<double*>(smem2 + 4 * (size_t)LE);
+#define GEO2(f) (*reinterpret_cast<const double2*>(geo + (f) * K2_T + 2 * threadIdx.x))
 
   if (threadIdx.x < nw) {
     double sl, cl, sb, cb;
@@ -87,39 +90,60 @@ __global__ void __launch_bounds__(K2_T, 3) k2_link_response(const K2Params p) {
     s[0] = -cb * cl; s[1] = -cb * sl; s[2] = -sb;  // k
     s[3] = sl;       s[4] = -cl;      s[5] = 0.0;  // u
     s[6] = -sb * cl; s[7] = -sb * sl; s[8] = cb;   // v
+    double Dc0 = 0.0;
+    if (KIND == 1) {
+      double sM, cM;
+      sincos_d(fma(p.orb.w, fma((double)n0, p.dt, p.t0) - p.orb.t_ref, -p.orb.phase0), sM, cM);
+      Dc0 = p.orb.a_over_c * p.inv_dt * fma(s[0], cM, s[1] * sM);
+    }
+    Kc[threadIdx.x] = __double2int_rn(Dc0);
   }
+  __syncthreads();
 
-  // ---- walker-independent geometry of this thread's sample, kept in registers
-  const long long n = n0 + threadIdx.x;
-  const bool in_grid = n < p.N;
-  const bool active = n >= R && n < p.N - R;
-  // geo[f][thread]: 0,1 common 1 AU delay per unit k (samples); 2..10 spacecraft offsets as
-  // delays per unit k (samples); 11..19 arm unit vectors (arm a: link_s(a) -> link_r(a));
-  // 20..22 / 23..25 light travel times of links +a / -a (samples)
-  double* geo = reinterpret_cast<double*>(tiles + 2 * (size_t)tile_len) + threadIdx.x;
-#define GEO(f) geo[(f) * K2_T]
-  {
+  auto prefetch = [&](int w, int buf) {
+    const double* hp = p.hplus + (size_t)(w0 + w) * p.N;
+    const double* hc = p.hcross + (size_t)(w0 + w) * p.N;
+    double2* dst = smem2 + (size_t)buf * 2 * LE;
+    const long long g0 = n0 - Kc[w] - p.halo;
+    for (int i = threadIdx.x; i < tile_len; i += K2_THREADS) {
+      const long long g = g0 + i;
+      const bool ok = g >= 0 && g < p.N;
+      const long long src = ok ? g : 0;
+      double2* d = dst + (i & 1) * LE + (i >> 1);
+      k2_cp_async8_zfill(&d->x, hp + src, ok);
+      k2_cp_async8_zfill(&d->y, hc + src, ok);
+    }
+    asm volatile("cp.async.commit_group;\n" ::);
+  };
+  prefetch(0, 0);
+
+  // ---- walker-independent geometry of this thread's two samples -> geo[field][sample]
+  const long long na = n0 + 2 * threadIdx.x;
+#pragma unroll 1
+  for (int c = 0; c < 2; ++c) {
+    double* gq = geo + 2 * threadIdx.x + c;
     double d[3][3], cM, sM;
-    orbit_offsets(p.orb, fma((double)n, p.dt, p.t0), d, cM, sM);
+    orbit_offsets(p.orb, fma((double)(na + c), p.dt, p.t0), d, cM, sM);
     const double sc = p.inv_dt / C_LIGHT;
-    GEO(0) = p.orb.a_over_c * p.inv_dt * cM;
-    GEO(1) = p.orb.a_over_c * p.inv_dt * sM;
+    gq[0 * K2_T] = p.orb.a_over_c * p.inv_dt * cM;   // common 1 AU delay per unit k (samples)
+    gq[1 * K2_T] = p.orb.a_over_c * p.inv_dt * sM;
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) GEO(2 + 3 * k + j) = d[k][j] * sc;
+      for (int j = 0; j < 3; ++j) gq[(2 + 3 * k + j) * K2_T] = d[k][j] * sc;  // offsets as delays per unit k
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       const int s = link_s(a), r = link_r(a);
       const double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
-      const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
-      const double inv = 1.0 / len;
-      GEO(11 + 3 * a) = dx * inv; GEO(12 + 3 * a) = dy * inv; GEO(13 + 3 * a) = dz * inv;
-      GEO(20 + a) = KIND == 0 ? p.orb.L[a] * p.inv_dt : len * sc;
-      GEO(23 + a) = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : len * sc;
+      const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) * sc;  // arm length in samples
+      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : len;        // light travel time of link +a
+      gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : len;    // of link -a
+      gq[(17 + a) * K2_T] = 1.0 / len;  // n_a = (offset_r - offset_s) / len
     }
   }
-  const int n_rel = threadIdx.x + R;
+  const bool act[2] = {na >= R && na < p.N - R, na + 1 >= R && na + 1 < p.N - R};
+  const bool vec_store = (p.N & 1) == 0;
+  const int elo = p.half - 1, ehi = tile_len - 2 - p.half;
 
   for (int w = 0; w < nw; ++w) {
     const int buf = w & 1;
@@ -129,45 +153,80 @@ __global__ void __launch_bounds__(K2_T, 3) k2_link_response(const K2Params p) {
     } else {
       asm volatile("cp.async.wait_group 0;\n" ::);
     }
-    __syncthreads();  // tile of walker w (and, first time round, sky[]) visible to everyone
-    double* yb = p.y + (size_t)(w0 + w) * 6 * p.N + n;
-    if (active) {
-      const double2* tile = tiles + (size_t)buf * tile_len;
+    __syncthreads();  // tile of walker w (and, first time round, geo[]) visible to everyone
+    double* yb = p.y + (size_t)(w0 + w) * 6 * p.N + na;
+    double yo[6][2];
+    if (act[0] || act[1]) {
+      const double2* xe = smem2 + (size_t)buf * 2 * LE;
+      const double2* xo = xe + LE;
+      const int ea0 = 2 * threadIdx.x + p.halo + Kc[w];
       const double* s = sky[w];
       const double kx = s[0], ky = s[1], kz = s[2];
-      const double ux = s[3], uy = s[4], uz = s[5];
+      const double ux = s[3], uy = s[4];  // uz = 0
       const double vx = s[6], vy = s[7], vz = s[8];
-      const double Dc = fma(kx, GEO(0), ky * GEO(1));
-      double Dk[3], hpr[3], hcr[3];
+      double Dc[2], kd[3][2], ud[3][2], vd[3][2];
+      {
+        const double2 g0 = GEO2(0), g1 = GEO2(1);
+        Dc[0] = fma(kx, g0.x, ky * g1.x);
+        Dc[1] = fma(kx, g0.y, ky * g1.y);
+      }
 #pragma unroll
-      for (int k = 0; k < 3; ++k) Dk[k] = fma(kx, GEO(2 + 3 * k), fma(ky, GEO(3 + 3 * k), kz * GEO(4 + 3 * k)));
+      for (int k = 0; k < 3; ++k) {
+        const double2 dx = GEO2(2 + 3 * k), dy = GEO2(3 + 3 * k), dz = GEO2(4 + 3 * k);
+        kd[k][0] = fma(kx, dx.x, fma(ky, dy.x, kz * dz.x));
+        kd[k][1] = fma(kx, dx.y, fma(ky, dy.y, kz * dz.y));
+        ud[k][0] = fma(ux, dx.x, uy * dy.x);
+        ud[k][1] = fma(ux, dx.y, uy * dy.y);
+        vd[k][0] = fma(vx, dx.x, fma(vy, dy.x, vz * dz.x));
+        vd[k][1] = fma(vx, dx.y, fma(vy, dy.y, vz * dz.y));
+      }
       // the three reception-time reads h(t - k.r_r/c)
+      double hpr[3][2], hcr[3][2];
 #pragma unroll
-      for (int k = 0; k < 3; ++k) read_pair<HT>(tile, tile_len, n_rel, Dc, Dk[k], p, hpr[k], hcr[k]);
+      for (int k = 0; k < 3; ++k) read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd[k][0], kd[k][1], p, hpr[k], hcr[k]);
       // three arms; links a and -a share x+, xx and have opposite n
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         const int sd = link_s(a), rc = link_r(a);
-        const double nx = GEO(11 + 3 * a), ny = GEO(12 + 3 * a), nz = GEO(13 + 3 * a);
-        const double un = fma(ux, nx, fma(uy, ny, uz * nz));
-        const double vn = fma(vx, nx, fma(vy, ny, vz * nz));
-        const double kn = fma(kx, nx, fma(ky, ny, kz * nz));
-        const double xp = fma(un, un, -vn * vn);
-        const double xc2 = 2.0 * un * vn;
-        const double om = 1.0 - kn, opl = 1.0 + kn;
-        const double inv = 0.5 / (om * opl);  // 1/(2(1-kn)) = (1+kn) inv, 1/(2(1+kn)) = (1-kn) inv
-        double hps, hcs;
-        read_pair<HT>(tile, tile_len, n_rel, Dc, GEO(20 + a) + Dk[sd], p, hps, hcs);   // link +a: sd -> rc
-        yb[(size_t)a * p.N] = fma(xp, hps - hpr[rc], xc2 * (hcs - hcr[rc])) * (opl * inv);
-        read_pair<HT>(tile, tile_len, n_rel, Dc, GEO(23 + a) + Dk[rc], p, hps, hcs);   // link -a: rc -> sd
-        yb[(size_t)(a + 3) * p.N] = fma(xp, hps - hpr[sd], xc2 * (hcs - hcr[sd])) * (om * inv);
-      }
-    } else if (in_grid) {
+        const double2 Lp = GEO2(11 + a), Lm = GEO2(14 + a), il = GEO2(17 + a);
+        const double ila[2] = {il.x, il.y};
+        double xp[2], xc2[2], fp[2], fm[2];
 #pragma unroll
-      for (int l = 0; l < 6; ++l) yb[(size_t)l * p.N] = 0.0;
+        for (int c = 0; c < 2; ++c) {
+          const double un = (ud[rc][c] - ud[sd][c]) * ila[c];
+          const double vn = (vd[rc][c] - vd[sd][c]) * ila[c];
+          const double kn = (kd[rc][c] - kd[sd][c]) * ila[c];
+          xp[c] = fma(un, un, -vn * vn);
+          xc2[c] = 2.0 * un * vn;
+          const double om = 1.0 - kn, opl = 1.0 + kn;
+          const double inv = 0.5 / (om * opl);  // 1/(2(1-kn)) = (1+kn) inv, 1/(2(1+kn)) = (1-kn) inv
+          fp[c] = opl * inv;
+          fm[c] = om * inv;
+        }
+        double hps[2], hcs[2];
+        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lp.x + kd[sd][0], Lp.y + kd[sd][1], p, hps, hcs);  // link +a: sd -> rc
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          yo[a][c] = fma(xp[c], hps[c] - hpr[rc][c], xc2[c] * (hcs[c] - hcr[rc][c])) * fp[c];
+        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lm.x + kd[rc][0], Lm.y + kd[rc][1], p, hps, hcs);  // link -a: rc -> sd
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          yo[a + 3][c] = fma(xp[c], hps[c] - hpr[sd][c], xc2[c] * (hcs[c] - hcr[sd][c])) * fm[c];
+      }
     }
-    __syncthreads();  // everyone is done with tiles[buf] before walker w+2 is prefetched into it
+#pragma unroll
+    for (int l = 0; l < 6; ++l) {
+      const double v0 = act[0] ? yo[l][0] : 0.0, v1 = act[1] ? yo[l][1] : 0.0;
+      if (vec_store) {
+        if (na < p.N) *reinterpret_cast<double2*>(yb + (size_t)l * p.N) = make_double2(v0, v1);
+      } else {
+        if (na < p.N) yb[(size_t)l * p.N] = v0;
+        if (na + 1 < p.N) yb[(size_t)l * p.N + 1] = v1;
+      }
+    }
+    __syncthreads();  // everyone is done with buffer `buf` before walker w+2 is prefetched into it
   }
+#undef GEO2
 }
 
 // A12: y_l[n] = p(n - L_l(t_n)/dt) - p[n].  Small helper kernel, reads p from global memory.
@@ -201,21 +260,18 @@ __global__ void __launch_bounds__(256) k_laser_links(const LaserParams q) {
   }
 }
 
-#undef GEO
-
 template <int HT>
 static int launch_k2(const K2Params& p, cudaStream_t st) {
-  const size_t smem = (size_t)2 * (K2_T + 2 * p.margin) * sizeof(double2) + (size_t)26 * K2_T * sizeof(double);
-  if (smem > 100 * 1024) return set_error(LISA_TD_EINVAL, "link_response: margin_y too large for the shared-memory tile");
+  const int tile_len = K2_T + 2 * p.halo;
+  const size_t smem = (size_t)4 * ((tile_len + 1) / 2 + 1) * sizeof(double2) + (size_t)K2_NGEO * K2_T * sizeof(double);
+  if (smem > 220 * 1024) return set_error(LISA_TD_EINVAL, "link_response: delay spread of %d samples too large for the shared-memory tile", p.halo);
   dim3 grid((unsigned)((p.N + K2_T - 1) / K2_T), (unsigned)((p.B + p.group - 1) / p.group));
   if (p.orb.kind == 0) {
-    if (smem > 48 * 1024)
-      LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k2_link_response<HT, 0><<<grid, K2_T, smem, st>>>(p);
+    LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k2_link_response<HT, 0><<<grid, K2_THREADS, smem, st>>>(p);
   } else {
-    if (smem > 48 * 1024)
-      LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k2_link_response<HT, 1><<<grid, K2_T, smem, st>>>(p);
+    LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k2_link_response<HT, 1><<<grid, K2_THREADS, smem, st>>>(p);
   }
   LISA_LAUNCH_CHECK("k2_link_response");
   return LISA_TD_OK;
@@ -232,7 +288,8 @@ int run_link_response(int B, long long N, double t0, double dt, int order, long 
   p.hplus = hplus; p.hcross = hcross; p.lambda = lambda; p.beta_sky = beta_sky; p.y = y;
   p.orb = orb;
   p.group = B < K2_G ? B : K2_G;
-  make_lagw(order, &p.lw);
+  // |K - Kc| <= |Dl| + drift of Dc over the tile + 1.5; the pair window adds half + 1
+  p.halo = (int)ceil((orb.max_off_over_c + orb.max_L) / dt + orb.a_over_c * orb.w * K2_T + 1.5) + p.half + 2;
   make_lags(order, &p.ls);
   if (!g_force_generic) {
     switch (p.half) {
