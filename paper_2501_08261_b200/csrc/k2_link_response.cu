@@ -155,7 +155,17 @@ __global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params
     }
     __syncthreads();  // tile of walker w (and, first time round, geo[]) visible to everyone
     double* yb = p.y + (size_t)(w0 + w) * 6 * p.N + na;
-    double yo[6][2];
+    auto store2 = [&](int l, double v0, double v1) {
+      double* dst = yb + (size_t)l * p.N;
+      v0 = act[0] ? v0 : 0.0;
+      v1 = act[1] ? v1 : 0.0;
+      if (vec_store) {
+        if (na < p.N) *reinterpret_cast<double2*>(dst) = make_double2(v0, v1);
+      } else {
+        if (na < p.N) dst[0] = v0;
+        if (na + 1 < p.N) dst[1] = v1;
+      }
+    };
     if (act[0] || act[1]) {
       const double2* xe = smem2 + (size_t)buf * 2 * LE;
       const double2* xo = xe + LE;
@@ -164,12 +174,17 @@ __global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params
       const double kx = s[0], ky = s[1], kz = s[2];
       const double ux = s[3], uy = s[4];  // uz = 0
       const double vx = s[6], vy = s[7], vz = s[8];
-      double Dc[2], kd[3][2], ud[3][2], vd[3][2];
+      double Dc[2];
       {
         const double2 g0 = GEO2(0), g1 = GEO2(1);
         Dc[0] = fma(kx, g0.x, ky * g1.x);
         Dc[1] = fma(kx, g0.y, ky * g1.y);
       }
+      // per spacecraft slot: k.offset, u.offset, v.offset (samples) and the reception-time
+      // reads h(t - k.r_r/c).  The loops below are NOT unrolled (the unrolled body overflowed
+      // the instruction cache); instead the three slots are rotated after every pass, so the
+      // loop body always addresses the same registers.
+      double kd[3][2], ud[3][2], vd[3][2], hpr[3][2], hcr[3][2];
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
         const double2 dx = GEO2(2 + 3 * k), dy = GEO2(3 + 3 * k), dz = GEO2(4 + 3 * k);
@@ -179,23 +194,32 @@ __global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params
         ud[k][1] = fma(ux, dx.y, uy * dy.y);
         vd[k][0] = fma(vx, dx.x, fma(vy, dy.x, vz * dz.x));
         vd[k][1] = fma(vx, dx.y, fma(vy, dy.y, vz * dz.y));
+        hpr[k][0] = hpr[k][1] = hcr[k][0] = hcr[k][1] = 0.0;
       }
-      // the three reception-time reads h(t - k.r_r/c)
-      double hpr[3][2], hcr[3][2];
-#pragma unroll
-      for (int k = 0; k < 3; ++k) read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd[k][0], kd[k][1], p, hpr[k], hcr[k]);
-      // three arms; links a and -a share x+, xx and have opposite n
-#pragma unroll
+#define ROT3(x)                                                  \
+  do {                                                           \
+    const double t0_ = x[0][0], t1_ = x[0][1];                   \
+    x[0][0] = x[1][0]; x[0][1] = x[1][1];                        \
+    x[1][0] = x[2][0]; x[1][1] = x[2][1];                        \
+    x[2][0] = t0_; x[2][1] = t1_;                                \
+  } while (0)
+#pragma unroll 1
+      for (int k = 0; k < 3; ++k) {  // slot 0 holds spacecraft k
+        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd[0][0], kd[0][1], p, hpr[0], hcr[0]);
+        ROT3(kd); ROT3(ud); ROT3(vd); ROT3(hpr); ROT3(hcr);
+      }
+      // three arms; links a and -a share x+, xx and have opposite n.  Arm a joins spacecraft
+      // link_s(a) = a+2 and link_r(a) = a+1 (mod 3): after a rotations they sit in slots 2, 1.
+#pragma unroll 1
       for (int a = 0; a < 3; ++a) {
-        const int sd = link_s(a), rc = link_r(a);
         const double2 Lp = GEO2(11 + a), Lm = GEO2(14 + a), il = GEO2(17 + a);
         const double ila[2] = {il.x, il.y};
         double xp[2], xc2[2], fp[2], fm[2];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-          const double un = (ud[rc][c] - ud[sd][c]) * ila[c];
-          const double vn = (vd[rc][c] - vd[sd][c]) * ila[c];
-          const double kn = (kd[rc][c] - kd[sd][c]) * ila[c];
+          const double un = (ud[1][c] - ud[2][c]) * ila[c];
+          const double vn = (vd[1][c] - vd[2][c]) * ila[c];
+          const double kn = (kd[1][c] - kd[2][c]) * ila[c];
           xp[c] = fma(un, un, -vn * vn);
           xc2[c] = 2.0 * un * vn;
           const double om = 1.0 - kn, opl = 1.0 + kn;
@@ -204,25 +228,18 @@ __global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params
           fm[c] = om * inv;
         }
         double hps[2], hcs[2];
-        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lp.x + kd[sd][0], Lp.y + kd[sd][1], p, hps, hcs);  // link +a: sd -> rc
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-          yo[a][c] = fma(xp[c], hps[c] - hpr[rc][c], xc2[c] * (hcs[c] - hcr[rc][c])) * fp[c];
-        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lm.x + kd[rc][0], Lm.y + kd[rc][1], p, hps, hcs);  // link -a: rc -> sd
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-          yo[a + 3][c] = fma(xp[c], hps[c] - hpr[sd][c], xc2[c] * (hcs[c] - hcr[sd][c])) * fm[c];
+        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lp.x + kd[2][0], Lp.y + kd[2][1], p, hps, hcs);  // link +a: s -> r
+        store2(a, fma(xp[0], hps[0] - hpr[1][0], xc2[0] * (hcs[0] - hcr[1][0])) * fp[0],
+               fma(xp[1], hps[1] - hpr[1][1], xc2[1] * (hcs[1] - hcr[1][1])) * fp[1]);
+        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lm.x + kd[1][0], Lm.y + kd[1][1], p, hps, hcs);  // link -a: r -> s
+        store2(a + 3, fma(xp[0], hps[0] - hpr[2][0], xc2[0] * (hcs[0] - hcr[2][0])) * fm[0],
+               fma(xp[1], hps[1] - hpr[2][1], xc2[1] * (hcs[1] - hcr[2][1])) * fm[1]);
+        ROT3(kd); ROT3(ud); ROT3(vd); ROT3(hpr); ROT3(hcr);
       }
-    }
+#undef ROT3
+    } else {
 #pragma unroll
-    for (int l = 0; l < 6; ++l) {
-      const double v0 = act[0] ? yo[l][0] : 0.0, v1 = act[1] ? yo[l][1] : 0.0;
-      if (vec_store) {
-        if (na < p.N) *reinterpret_cast<double2*>(yb + (size_t)l * p.N) = make_double2(v0, v1);
-      } else {
-        if (na < p.N) yb[(size_t)l * p.N] = v0;
-        if (na + 1 < p.N) yb[(size_t)l * p.N + 1] = v1;
-      }
+      for (int l = 0; l < 6; ++l) store2(l, 0.0, 0.0);
     }
     __syncthreads();  // everyone is done with buffer `buf` before walker w+2 is prefetched into it
   }
