@@ -11,6 +11,9 @@
 // once per tile instead of once per walker, and 16x32 taps shrink to 4xWIN.
 //
 // A plain one-thread-per-(walker, sample) kernel covers every other order / cadence.
+#include <cuda.h>
+#include <string.h>
+
 #include "common.cuh"
 
 namespace lisa {
@@ -168,9 +171,10 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
 // per 8 FMA instead of one per FMA (the previous SIMT version was shared-memory bound at 22 %
 // FP64-pipe activity).  Walkers stream through shared memory in chunks of 16 (cp.async,
 // double buffered); X,Y,Z of a chunk meet in shared memory for the A,E,T combination.
-constexpr int K3_TS = 32;                  // output samples per block
+constexpr int K3_TS = 32;                  // output samples per block (two 8-row MMA blocks)
 constexpr int K3_PAIRS = 12;               // (channel, series) pairs
-constexpr int K3_THREADS = 32 * K3_PAIRS;  // 12 warps
+constexpr int K3_THREADS = K3_TS * K3_PAIRS;  // phase 1: thread = (pair, sample); phase 2: warp = (channel, row block)
+constexpr int K3_RB = K3_TS / 8;           // 8-row blocks per tile
 constexpr int K3_WC = 16;                  // walkers per shared-memory chunk (two MMA N-blocks)
 constexpr int K3_XS = K3_WC + 1;           // row stride of the X,Y,Z exchange buffer
 
@@ -183,6 +187,39 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int NKEEP>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP));
+}
+// TMA (bulk async copy) of one contiguous run of global memory into shared memory, completion
+// counted in bytes on an mbarrier.  dst, src and bytes must be multiples of 16.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+// One 2-D tiled TMA copy: box (TW samples x rows) at coordinates (c0 = sample, c1 = row) of the
+// [B*6][N] y matrix; samples / rows outside the matrix arrive as zeros.
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* b) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(smem_u32(dst)),
+      "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(b))
+      : "memory");
+}
+// Spin on test_wait (try_wait suspends the warp for a system-dependent time; with one block per
+// SM every warp waits for the same tile, and late wake-ups showed up as barrier stalls).
+__device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(b)), "r"(parity)
+        : "memory");
+  } while (!done);
 }
 // D(8x8) += A(8x4, row) * B(4x8, col), fp64.  Lane l holds A[l/4][l%4], B[l%4][l/4] and
 // D[l/4][2(l%4) + {0,1}].
@@ -226,7 +263,8 @@ struct K3Geom {
   static constexpr int KCAP = WIN - 2 * H;            // largest integer delay the window holds
   static constexpr int LOW = -(KCAP + H - 1);         // offset of stencil tap 0 relative to n
   static constexpr int KSTEPS = (WIN + 7 + 3) / 4;    // k-steps of one 8-sample row block
-  static constexpr int TWMIN = 24 + 4 * KSTEPS;       // y samples a block touches per series
+  static constexpr int PAD = (LOW % 2 != 0) ? 1 : 0;  // the tile starts at the even sample n0 + LOW - PAD (16-byte aligned rows)
+  static constexpr int TWMIN = K3_TS - 8 + 4 * KSTEPS + PAD;  // y samples a block touches per series
   static constexpr int TW = TWMIN + ((2 - TWMIN % 4) + 4) % 4;  // == 2 mod 4: walker stride 6 TW == 4 or 12 mod 16
   static constexpr int CS = ((WIN + 2) / 8) * 8 + 5;  // odd, >= WIN, (CS-1) == 4 mod 8: conflict-free fragment reads
   static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
@@ -237,11 +275,14 @@ struct K3Geom {
 };
 
 template <int H, int WIN>
-__global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
+__global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
+    k3_tdi_mma(const K3Params p, const __grid_constant__ CUtensorMap tmap, const int use_tma) {
   using G = K3Geom<H, WIN>;
-  constexpr int KCAP = G::KCAP, LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, CS = G::CS;
+  constexpr int KCAP = G::KCAP, LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, CS = G::CS, PAD = G::PAD;
+  constexpr int NWARPS = K3_THREADS / 32;
+  __shared__ __align__(8) uint64_t mbar[2];  // one per walker-chunk buffer (TMA completion)
   static_assert(CS >= WIN && (CS & 1), "stencil row stride");
-  extern __shared__ double smem[];
+  extern __shared__ __align__(128) double smem[];
   double* ys = smem;                    // [2][WC][6][TW]   (phase 2)
   double* cbuf = smem;                  // [12][32][CS]     (phase 1, aliased)
   double* xs = smem + G::UNION;         // [3][32][XS]
@@ -250,12 +291,17 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
   const int wid = threadIdx.x >> 5;
   const long long n0 = (long long)blockIdx.x * K3_TS;
 
-  // ---- phase 1a: light travel times of the 32 samples
-  if (wid == 0) {
+  if (threadIdx.x == 0) {
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  // ---- phase 1a: light travel times of the tile's samples
+  if (threadIdx.x < K3_TS) {
     double L[6];
-    orbit_arm_times(p.orb, fma((double)(n0 + lane), p.dt, p.t0), L);
+    orbit_arm_times(p.orb, fma((double)(n0 + threadIdx.x), p.dt, p.t0), L);
 #pragma unroll
-    for (int l = 0; l < 6; ++l) Ls[lane * 6 + l] = L[l];
+    for (int l = 0; l < 6; ++l) Ls[threadIdx.x * 6 + l] = L[l];
   }
   __syncthreads();
   // ---- phase 1b: merged stencil of (pair = wid, sample = lane)
@@ -263,12 +309,13 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
     double C[WIN];
 #pragma unroll
     for (int i = 0; i < WIN; ++i) C[i] = 0.0;
-    const K3Pair& pr = p.pair[wid];
-    const long long n = n0 + lane;
+    const int pi = threadIdx.x / K3_TS, sm = threadIdx.x % K3_TS;  // pair, sample
+    const K3Pair& pr = p.pair[pi];
+    const long long n = n0 + sm;
     if (n >= p.margin_lo && n < p.N - p.margin_hi) {
       double L[6];
 #pragma unroll
-      for (int l = 0; l < 6; ++l) L[l] = Ls[lane * 6 + l];
+      for (int l = 0; l < 6; ++l) L[l] = Ls[sm * 6 + l];
       for (int k = 0; k < pr.n_terms; ++k) {
         const double D = term_delay(pr.t[k], L, p.inv_dt);
         const double Kf = ceil(D);
@@ -278,13 +325,13 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
         TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.lw);
       }
     }
-    double* dst = cbuf + (size_t)(wid * K3_TS + lane) * CS;
+    double* dst = cbuf + (size_t)(pi * K3_TS + sm) * CS;
 #pragma unroll
     for (int i = 0; i < WIN; ++i) dst[i] = C[i];
   }
   __syncthreads();
   // ---- phase 1c: A fragments of (channel ch, row block rb): 4 pairs x KSTEPS values
-  const int ch = wid >> 2, rb = wid & 3;
+  const int ch = wid / K3_RB, rb = wid % K3_RB;
   const int r = lane >> 2, kk = lane & 3;
   double A[4][KSTEPS];
   int ser[4];
@@ -302,30 +349,47 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
 
   // ---- phase 2: stream walkers
   const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
+  // Walker chunks arrive by TMA: ONE 2-D tiled copy per chunk (box = TW samples x 96 rows of the
+  // [B*6][N] matrix; parts of the box outside the matrix are zero-filled by the hardware, which
+  // covers both the grid edges and a ragged last chunk), completion counted on the buffer's
+  // mbarrier.  The tensor map needs 16-byte row strides, so odd N takes the zero-filling
+  // cp.async path instead.
+  const long long g0 = n0 + LOW - PAD;
   auto prefetch = [&](int chunk, int buf) {
     double* dst = ys + (size_t)buf * G::YBUF;
-    for (int e = threadIdx.x; e < G::YBUF; e += K3_THREADS) {
-      const int row = e / TW, i = e - row * TW;
-      const int w = chunk * K3_WC + row / 6;
-      const long long g = n0 + LOW + i;
-      const bool ok = (w < p.B) && g >= 0 && g < p.N;
-      const size_t src = ok ? ((size_t)w * 6 + (row % 6)) * p.N + g : 0;
-      cp_async8_zfill(dst + e, p.y + src, ok);
+    if (use_tma) {
+      if (threadIdx.x == 0) {
+        mbar_arrive_expect_tx(&mbar[buf], (unsigned)(G::YBUF * sizeof(double)));
+        tma_load_2d(dst, &tmap, (int)g0, chunk * K3_WC * 6, &mbar[buf]);
+      }
+    } else {
+      const int nrows = min(K3_WC, p.B - chunk * K3_WC) * 6;
+      const double* src0 = p.y + (size_t)chunk * K3_WC * 6 * p.N + g0;
+      for (int row = wid; row < K3_WC * 6; row += NWARPS) {
+        const double* src = src0 + (size_t)row * p.N;
+        for (int i = lane; i < TW; i += 32) {
+          const long long g = g0 + i;
+          const bool ok = row < nrows && g >= 0 && g < p.N;
+          cp_async8_zfill(dst + row * TW + i, ok ? src + i : p.y, ok);
+        }
+      }
+      cp_async_commit();
     }
-    cp_async_commit();
   };
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // cbuf (generic writes) -> ys (TMA writes)
   prefetch(0, 0);
   for (int c = 0; c < n_chunks; ++c) {
     const int buf = c & 1;
-    if (c + 1 < n_chunks) {
-      prefetch(c + 1, buf ^ 1);
-      cp_async_wait<1>();
+    if (c + 1 < n_chunks) prefetch(c + 1, buf ^ 1);
+    if (use_tma) {
+      mbar_wait(&mbar[buf], (unsigned)((c >> 1) & 1));
     } else {
-      cp_async_wait<0>();
+      if (c + 1 < n_chunks) cp_async_wait<1>();
+      else cp_async_wait<0>();
     }
     __syncthreads();  // chunk c landed; everyone is done with xs of chunk c-1
     // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
-    const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk;
+    const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
     double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -343,7 +407,7 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
     }
     __syncthreads();
     for (int e = threadIdx.x; e < K3_WC * 3 * K3_TS; e += K3_THREADS) {
-      const int ln = e & 31, o = (e >> 5) % 3, w = e / 96;
+      const int ln = e % K3_TS, o = (e / K3_TS) % 3, w = e / (3 * K3_TS);
       const int b = c * K3_WC + w;
       const long long nn = n0 + ln;
       if (b >= p.B || nn >= p.N) continue;
@@ -359,12 +423,42 @@ __global__ void __launch_bounds__(K3_THREADS, 1) k3_tdi_mma(const K3Params p) {
   }
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(ptr);
+  }
+  return fn;
+}
+
 template <int H, int WIN>
 static int launch_mma(const K3Params& p, cudaStream_t st) {
   using G = K3Geom<H, WIN>;
   static_assert(G::SMEM <= 227 * 1024, "k3_tdi_mma shared memory");
+  static_assert((G::YBUF * sizeof(double)) % 128 == 0, "TMA destination alignment");
+  CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  int use_tma = 0;
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (enc && (p.N & 1) == 0 && p.N < (1LL << 31)) {
+    const cuuint64_t gdim[2] = {(cuuint64_t)p.N, (cuuint64_t)p.B * 6};
+    const cuuint64_t gstr[1] = {(cuuint64_t)p.N * sizeof(double)};
+    const cuuint32_t box[2] = {(cuuint32_t)G::TW, (cuuint32_t)(K3_WC * 6)};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(p.y), gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    use_tma = r == CUDA_SUCCESS;
+  }
   LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-  k3_tdi_mma<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, G::SMEM, st>>>(p);
+  k3_tdi_mma<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, G::SMEM, st>>>(p, tmap, use_tma);
   LISA_LAUNCH_CHECK("k3_tdi_mma");
   return LISA_TD_OK;
 }
