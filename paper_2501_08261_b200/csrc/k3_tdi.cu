@@ -269,7 +269,7 @@ struct K3Geom {
   static constexpr int CS = ((WIN + 2) / 8) * 8 + 5;  // odd, >= WIN, (CS-1) == 4 mod 8: conflict-free fragment reads
   static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
   static constexpr int CBUF = K3_PAIRS * K3_TS * CS;  // doubles of the stencil staging area
-  static constexpr int XBUF = 3 * K3_TS * K3_XS;
+  static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange
   static constexpr int UNION = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
   static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
 };
@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
   extern __shared__ __align__(128) double smem[];
   double* ys = smem;                    // [2][WC][6][TW]   (phase 2)
   double* cbuf = smem;                  // [12][32][CS]     (phase 1, aliased)
-  double* xs = smem + G::UNION;         // [3][32][XS]
+  double* xs = smem + G::UNION;         // [2][3][TS][XS]
   double* Ls = xs + G::XBUF;            // [32][6]
   const int lane = threadIdx.x & 31;
   const int wid = threadIdx.x >> 5;
@@ -387,7 +387,11 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
       if (c + 1 < n_chunks) cp_async_wait<1>();
       else cp_async_wait<0>();
     }
-    __syncthreads();  // chunk c landed; everyone is done with xs of chunk c-1
+    // TMA path: the mbarrier wait makes the tile visible to each waiting thread, and the
+    // X,Y,Z exchange buffer alternates, so ONE barrier per chunk (after the MMAs) is enough:
+    // warps that finish their stores early start the next chunk's MMAs.
+    if (!use_tma) __syncthreads();  // cp.async path: other threads' copies become visible here
+    double* xsc = xs + (size_t)buf * (3 * K3_TS * K3_XS);
     // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
     const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
     double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
@@ -402,23 +406,41 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
       }
     }
     {
-      double* xr = xs + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
+      double* xr = xsc + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
       xr[0] = d00; xr[1] = d01; xr[8] = d10; xr[9] = d11;
     }
-    __syncthreads();
-    for (int e = threadIdx.x; e < K3_WC * 3 * K3_TS; e += K3_THREADS) {
-      const int ln = e % K3_TS, o = (e / K3_TS) % 3, w = e / (3 * K3_TS);
+    __syncthreads();  // X,Y,Z of chunk c complete; every warp is done reading y buffer `buf`
+    // thread = (walker, two adjacent samples): X,Y,Z -> the three output channels, one 16-byte
+    // store per channel
+    const bool vec = (p.N & 1) == 0;
+    for (int e = threadIdx.x; e < K3_WC * (K3_TS / 2); e += K3_THREADS) {
+      const int l2 = e % (K3_TS / 2), w = e / (K3_TS / 2);
       const int b = c * K3_WC + w;
-      const long long nn = n0 + ln;
+      const long long nn = n0 + 2 * l2;
       if (b >= p.B || nn >= p.N) continue;
-      const double X = xs[(0 * K3_TS + ln) * K3_XS + w];
-      const double Y = xs[(1 * K3_TS + ln) * K3_XS + w];
-      const double Z = xs[(2 * K3_TS + ln) * K3_XS + w];
-      double out[3];
-      combine_out(p.out_kind, X, Y, Z, out);
-      double v = o == 0 ? out[0] : (o == 1 ? out[1] : out[2]);
-      if (nn < p.margin_lo || nn >= p.N - p.margin_hi) v = 0.0;
-      p.tdi[((size_t)b * 3 + o) * p.N + nn] = v;
+      double v[3][2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int ln = 2 * l2 + h;
+        const double X = xsc[(0 * K3_TS + ln) * K3_XS + w];
+        const double Y = xsc[(1 * K3_TS + ln) * K3_XS + w];
+        const double Z = xsc[(2 * K3_TS + ln) * K3_XS + w];
+        double out[3];
+        combine_out(p.out_kind, X, Y, Z, out);
+        const bool zero = nn + h < p.margin_lo || nn + h >= p.N - p.margin_hi;
+#pragma unroll
+        for (int o = 0; o < 3; ++o) v[o][h] = zero ? 0.0 : out[o];
+      }
+#pragma unroll
+      for (int o = 0; o < 3; ++o) {
+        double* dst = p.tdi + ((size_t)b * 3 + o) * p.N + nn;
+        if (vec) {
+          *reinterpret_cast<double2*>(dst) = make_double2(v[o][0], v[o][1]);
+        } else {
+          dst[0] = v[o][0];
+          if (nn + 1 < p.N) dst[1] = v[o][1];
+        }
+      }
     }
   }
 }
