@@ -198,6 +198,22 @@ __device__ __forceinline__ K1Pre k1_pre(const quat& q) {
   return r;
 }
 
+// V samples per thread (V = 2: adjacent samples, 16-byte loads and stores; needs even N).  All 13
+// input values of the thread are loaded BEFORE any arithmetic so that each thread has 13 x 8 V
+// bytes in flight (the first version interleaved loads with the sincos evaluations and sat on
+// the HBM latency: long_scoreboard 9.8 per issue at 52 % of HBM bandwidth).
+template <int V>
+__device__ __forceinline__ void k1_load(const double* __restrict__ ptr, size_t n, double (&out)[V]) {
+  if constexpr (V == 2) {
+    const double2 t = __ldg(reinterpret_cast<const double2*>(ptr + n));
+    out[0] = t.x;
+    out[1] = t.y;
+  } else {
+    out[0] = __ldg(ptr + n);
+  }
+}
+
+template <int V>
 __global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol_std5(const K1FastParams p) {
   __shared__ quat Qc;
   __shared__ double rot[2];
@@ -216,26 +232,39 @@ __global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol_std5(const K1FastP
   const size_t bN = (size_t)b * p.N;
   const double* amp = p.amp + bN * p.n_modes;
   const double* pha = p.phase + bN * p.n_modes;
+  const long long n = ((long long)blockIdx.x * K1_THREADS + threadIdx.x) * V;
+  if (n >= p.N) return;
+  // ---- all loads first
+  double al[V], be[V], ga[V], am[5][V], ph[5][V];
+  if (p.twisted) {
+    k1_load<V>(p.alpha, bN + n, al);
+    k1_load<V>(p.beta, bN + n, be);
+    k1_load<V>(p.gamma, bN + n, ga);
+  }
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) am[k][v] = ph[k][v] = 0.0;
+    if (p.idx[k] >= 0) {
+      k1_load<V>(amp, (size_t)p.idx[k] * p.N + n, am[k]);
+      k1_load<V>(pha, (size_t)p.idx[k] * p.N + n, ph[k]);
+    }
+  }
   const quat qc = Qc;
   K1Pre pre = k1_pre(qc);
-  const long long n_base = (long long)blockIdx.x * (K1_THREADS * K1_PER_THREAD);
-#pragma unroll 1
-  for (int it = 0; it < K1_PER_THREAD; ++it) {
-    const long long n = n_base + it * K1_THREADS + threadIdx.x;
-    if (n >= p.N) break;
-    if (p.twisted) pre = k1_pre(quat_mul(quat_from_euler(p.alpha[bN + n], p.beta[bN + n], p.gamma[bN + n]), qc));
+  const double cc[5] = {p.c22, p.c21, p.c33, p.c44, p.c55};
+  double hp[V], hx[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    if (p.twisted) pre = k1_pre(quat_mul(quat_from_euler(al[v], be[v], ga[v]), qc));
     // h_k = a (cos phi - i sin phi), scaled by its constant
     cplx h[5];
-    const double cc[5] = {p.c22, p.c21, p.c33, p.c44, p.c55};
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
-      h[k] = {0.0, 0.0};
-      if (p.idx[k] >= 0) {
-        double s, c;
-        const double a = amp[(size_t)p.idx[k] * p.N + n] * cc[k];
-        sincos_d(pha[(size_t)p.idx[k] * p.N + n], s, c);
-        h[k] = {a * c, -a * s};
-      }
+      double s, c;
+      const double a = am[k][v] * cc[k];
+      sincos_d(ph[k][v], s, c);
+      h[k] = {a * c, -a * s};
     }
     // G = h22 + z (h33 + z (h44 + z h55))
     cplx g = cmul(pre.z, h[4]);
@@ -248,8 +277,15 @@ __global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol_std5(const K1FastP
     cplx u1 = cmul(pre.qa2, h[1]), u2 = cmul(pre.qb2, cconj(h[1]));
     cplx u = cmul(pre.qab, {u1.re + u2.re, u1.im + u2.im});
     const double Hre = (t1.re + t2.re) + u.re, Him = (t1.im + t2.im) + u.im;
-    p.hplus[bN + n] = fma(Hre, rot[0], -Him * rot[1]);
-    p.hcross[bN + n] = -fma(Hre, rot[1], Him * rot[0]);
+    hp[v] = fma(Hre, rot[0], -Him * rot[1]);
+    hx[v] = -fma(Hre, rot[1], Him * rot[0]);
+  }
+  if constexpr (V == 2) {
+    *reinterpret_cast<double2*>(p.hplus + bN + n) = make_double2(hp[0], hp[1]);
+    *reinterpret_cast<double2*>(p.hcross + bN + n) = make_double2(hx[0], hx[1]);
+  } else {
+    p.hplus[bN + n] = hp[0];
+    p.hcross[bN + n] = hx[0];
   }
 }
 
@@ -295,8 +331,13 @@ int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m
       f.B = B; f.N = N; f.n_modes = n_modes; f.twisted = alpha != nullptr; f.have_e0 = euler0 != nullptr;
       f.amp = amp; f.phase = phase; f.alpha = alpha; f.beta = beta; f.gamma = gamma;
       f.iota = iota; f.phi = phi; f.psi = psi; f.euler0 = euler0; f.hplus = hplus; f.hcross = hcross;
-      dim3 grid((unsigned)((N + K1_THREADS * K1_PER_THREAD - 1) / (K1_THREADS * K1_PER_THREAD)), (unsigned)B);
-      k1_modes_to_pol_std5<<<grid, K1_THREADS, 0, st>>>(f);
+      if ((N & 1) == 0) {
+        dim3 grid((unsigned)((N / 2 + K1_THREADS - 1) / K1_THREADS), (unsigned)B);
+        k1_modes_to_pol_std5<2><<<grid, K1_THREADS, 0, st>>>(f);
+      } else {
+        dim3 grid((unsigned)((N + K1_THREADS - 1) / K1_THREADS), (unsigned)B);
+        k1_modes_to_pol_std5<1><<<grid, K1_THREADS, 0, st>>>(f);
+      }
       LISA_LAUNCH_CHECK("k1_modes_to_pol_std5");
       return LISA_TD_OK;
     }

@@ -38,6 +38,7 @@ struct K3Params {
   double* tdi;
   OrbitDev orb;
   LagW lw;
+  LagS ls;
   K3Pair pair[12];  // [channel X,Y,Z][slot]
 };
 
@@ -229,33 +230,35 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "d"(a), "d"(b));
 }
 
-// Adds sgn * c_j(eps) into the merged stencil at compile-time offset OFF.
+// Adds sgn * c_j(eps) into the merged stencil at compile-time offset OFF (scaled weights,
+// common.cuh LagS: 7 fp64 ops per node pair + the two accumulations).
 template <int H, int WIN, int OFF>
-__device__ __forceinline__ void add_term_at(double (&C)[WIN], double eps, double sgn, const LagW& lw) {
+__device__ __forceinline__ void add_term_at(double (&C)[WIN], double eps, double sgn, const LagS& ls) {
   double P[H + 1];
   const double q = eps * (eps - 1.0);
-  P[1] = 1.0;
+  P[1] = ls.g * sgn;
 #pragma unroll
-  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
-  double S = sgn;
+  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * fma(ls.rho[k - 1], q, ls.rc[k - 1]);
+  double S = 1.0;
 #pragma unroll
   for (int k = H; k >= 1; --k) {
-    double a = (lw.w[k - 1] * P[k]) * S;
-    C[OFF + k + H - 1] = fma(a, eps + (double)(k - 1), C[OFF + k + H - 1]);
-    C[OFF + H - k] = fma(a, (double)k - eps, C[OFF + H - k]);
-    S *= q + (double)(k * (1 - k));
+    const double a = P[k] * S;
+    const double t = a * eps;
+    C[OFF + k + H - 1] += k == 1 ? t : fma(a, (double)(k - 1), t);
+    C[OFF + H - k] += fma(a, (double)k, -t);
+    if (k > 1) S *= fma(ls.rho[k - 1], q, ls.rc[k - 1]);
   }
 }
 template <int H, int WIN, int OFF>
 struct TermDispatch {
-  static __device__ __forceinline__ void run(double (&C)[WIN], int off, double eps, double sgn, const LagW& lw) {
-    if (off == OFF) add_term_at<H, WIN, OFF>(C, eps, sgn, lw);
-    else TermDispatch<H, WIN, OFF - 1>::run(C, off, eps, sgn, lw);
+  static __device__ __forceinline__ void run(double (&C)[WIN], int off, double eps, double sgn, const LagS& ls) {
+    if (off == OFF) add_term_at<H, WIN, OFF>(C, eps, sgn, ls);
+    else TermDispatch<H, WIN, OFF - 1>::run(C, off, eps, sgn, ls);
   }
 };
 template <int H, int WIN>
 struct TermDispatch<H, WIN, -1> {
-  static __device__ __forceinline__ void run(double (&)[WIN], int, double, double, const LagW&) {}
+  static __device__ __forceinline__ void run(double (&)[WIN], int, double, double, const LagS&) {}
 };
 
 template <int H, int WIN>
@@ -322,7 +325,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
         const double eps = Kf - D;
         int off = KCAP - (int)Kf;
         off = max(0, min(off, KCAP));
-        TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.lw);
+        TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.ls);
       }
     }
     double* dst = cbuf + (size_t)(pi * K3_TS + sm) * CS;
@@ -495,6 +498,7 @@ int run_tdi(int B, long long N, double t0, double dt, int order, int generation,
   p.half = (order + 1) / 2; p.generation = generation; p.out_kind = out_kind;
   p.margin_lo = margin_lo; p.margin_hi = margin_hi; p.y = y; p.tdi = tdi; p.orb = orb;
   make_lagw(order, &p.lw);
+  make_lags(order, &p.ls);
   build_pairs(generation, p.pair);
   const int nL = generation == 20 ? 7 : 3;
   const int kcap = (int)ceil(nL * orb.max_L / dt);
