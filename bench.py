@@ -38,17 +38,23 @@ ORDER = 31
 
 # Algorithmic fp64 work per walker-sample, in DFMA-equivalent
 # instructions (DADD, DMUL, DFMA each count 1; flops = 2 x this).
-K2_STENCIL = 18 * (ORDER + 1)          # 9 evaluation times x 2 polarisations x (p+1) taps
-K2_COEFF = 9 * (146)                   # 9 walker-dependent coefficient sets, 4.56 ops per tap
-K2_GEOM = 100                          # orbit, projections, delays
-K2_OPS = K2_STENCIL + K2_COEFF + K2_GEOM
+# 9 evaluation times, each a fused coefficient sweep + two dot products over (p+1)/2 node pairs
+# at 11 ops per pair (4 stencil FMAs + 7 for the two coefficients; the first pair saves one),
+# plus the per-walker projections, delays and six divisions-free link combinations.  The
+# walker-independent orbit evaluation is NOT credited.  The kernel executes 1762 (ncu).
+K2_SWEEP = 9 * (11 * (ORDER + 1) // 2 - 1)
+K2_GEOM = 150
+K2_OPS = K2_SWEEP + K2_GEOM            # 1725 ops = 3450 flop per walker-sample
 K2_BYTES = 16 + 48                     # h+,hx in, six links out
+# dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch at this workload
+# (ncu --set full capture summarised in profiles/r1_s3_k2_k3.md)
+K2_TRAFFIC_BYTES = 4.27e9
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=64, help=argparse.SUPPRESS)
@@ -69,7 +75,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -126,28 +132,30 @@ def dist_max(value: float, dist=None, device=None) -> float:
     return float(t.item())
 
 
-def oracle_sample_rate(inp, data, weight, kmin, kmax, window=1 << 14, cores=None):
+def oracle_sample_rate(inp, data, weight, kmin, kmax, window=None, walkers=1):
     """Time the fp64 CPU oracle, as it stands, on a bounded sample of the workload:
     S1..S3 for `window` output samples of walker 0, then S4+S5 (three full-length FFTs + inner
     product) for one walker.  Returns (evals_per_s, description, threads)."""
     from oracle.binding import Oracle
     orc = Oracle("d")
     N = inp["N"]
-    n = lambda k: None if inp[k] is None else inp[k][:1].contiguous().cpu().numpy()
-    lo = N // 2
+    window = N if window is None else min(window, N)
+    nwalk = min(walkers, int(inp["amp"].shape[0]))
+    n = lambda k: None if inp[k] is None else inp[k][:nwalk].contiguous().cpu().numpy()
+    lo = (N - window) // 2
     t0 = time.perf_counter()
     orc.chain(inp["l"], inp["m"], n("amp"), n("phase"), n("iota"), n("phi"), n("psi"), n("lam"), n("beta_sky"),
               inp["orbit"], inp["t0"], inp["dt"], inp["order"], inp["margin_y"], 20, 1, inp["margin_lo"],
               inp["margin_hi"], alpha=n("alpha"), beta=n("beta"), gamma=n("gamma"), n_lo=lo, n_hi=lo + window,
               want=("tdi",))
     t_win = time.perf_counter() - t0
-    tdi = np.zeros((1, 3, N))
-    tdi[0, :, lo:lo + window] = 1e-22
+    tdi = np.zeros((nwalk, 3, N))
+    tdi[:, :, lo:lo + window] = 1e-22
     t0 = time.perf_counter()
     orc.loglike(tdi, data, weight, kmin, kmax)
     t_fft = time.perf_counter() - t0
-    per_eval = t_win * (N / window) + t_fft
-    desc = (f"oracle (fp64 build, OpenMP) walker 0: S1-S3 on {window} of {N} output samples "
+    per_eval = (t_win * (N / window) + t_fft) / nwalk
+    desc = (f"oracle (fp64 build, OpenMP) on {nwalk} walker(s): S1-S3 on {window} of {N} output samples each "
             f"({t_win:.2f} s, scaled by N/{window}) + S4/S5 at full length ({t_fft:.2f} s)")
     return 1.0 / per_eval, desc, orc.num_threads()
 
@@ -168,7 +176,7 @@ def run_reference(args):
     data = np.zeros((3, N // 2 + 1, 2))
     vals, desc, threads = [], "", 1
     for i in range(args.warmup + args.steps):
-        v, desc, threads = oracle_sample_rate(inp, data, w, kmin, kmax, window=1 << 12)
+        v, desc, threads = oracle_sample_rate(inp, data, w, kmin, kmax, window=1 << 17)
         if i >= args.warmup:
             vals.append(v)
     value = float(len(vals) / sum(1.0 / v for v in vals))
@@ -293,7 +301,7 @@ def run_ours(args):
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
     roofline = {
         "kernel": "k2_link_response<16>", "bound": "alu", "achieved": achieved, "peak": dfma_peak_tflops,
-        "unit": "TFLOP/s", "frac": achieved / dfma_peak_tflops, "traffic": None,
+        "unit": "TFLOP/s", "frac": achieved / dfma_peak_tflops, "traffic": K2_TRAFFIC_BYTES,
         "peak_source": "DFMA probe measured in this run (lisa_td_probe_dfma, all SMs, ~1 s); nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2",
         "ops_per_walker_sample": K2_OPS, "ms_per_launch": k2_ms,
         "hbm_achieved_gbs": K2_BYTES * ws / (k2_ms * 1e-3) / 1e9,
@@ -333,8 +341,8 @@ def run_ours(args):
     # ---- the oracle beside it (bounded sample, host cores)
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        inp1 = {k: (v[:1].cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
-        v, desc, threads = oracle_sample_rate(inp1, data.cpu().numpy(), w_host, kmin, kmax)
+        inp1 = {k: (v[:2].cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
+        v, desc, threads = oracle_sample_rate(inp1, data.cpu().numpy(), w_host, kmin, kmax, walkers=2)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     line = {
