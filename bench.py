@@ -47,8 +47,8 @@ K2_GEOM = 150
 K2_OPS = K2_SWEEP + K2_GEOM            # 1725 ops = 3450 flop per walker-sample
 K2_BYTES = 16 + 48                     # h+,hx in, six links out
 # dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch at this workload
-# (ncu --set full capture summarised in profiles/r1_s3_k2_k3.md)
-K2_TRAFFIC_BYTES = 4.27e9
+# (ncu --set full capture summarised in profiles/r1_s3_k2_k3.md: 1.074 GB read + 3.188 GB written)
+K2_TRAFFIC_BYTES = 4.262e9
 
 
 def parse():
@@ -300,7 +300,7 @@ def run_ours(args):
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
     roofline = {
-        "kernel": "k2_link_response<16>", "bound": "alu", "achieved": achieved, "peak": dfma_peak_tflops,
+        "kernel": "k2_link_response<16,1>", "bound": "alu", "achieved": achieved, "peak": dfma_peak_tflops,
         "unit": "TFLOP/s", "frac": achieved / dfma_peak_tflops, "traffic": K2_TRAFFIC_BYTES,
         "peak_source": "DFMA probe measured in this run (lisa_td_probe_dfma, all SMs, ~1 s); nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2",
         "ops_per_walker_sample": K2_OPS, "ms_per_launch": k2_ms,
@@ -354,7 +354,7 @@ def run_ours(args):
                    "parallelism": f"walker-split x{world}, no collective"},
         "samples_per_s": value * N, "stage_ms": stage_ms, "roofline": roofline, "cpu_baseline": cpu_baseline,
         "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
-            "k1_modes_to_pol": 1, "k2_link_response": 1, "k3_tdi_merged": 1, "k5_inner_partial": 1,
+            "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "D2Z batch 192"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
     }
