@@ -18,8 +18,8 @@
 
 namespace lisa {
 
-constexpr int K2_T = 512;        // output samples per block
-constexpr int K2_THREADS = 256;  // two adjacent samples per thread
+constexpr int K2_T = 256;        // output samples per block
+constexpr int K2_THREADS = 128;  // two adjacent samples per thread
 constexpr int K2_G = 16;         // walkers per block (upper bound)
 constexpr int K2_NGEO = 20;      // geometry fields per sample
 
@@ -69,7 +69,7 @@ __device__ __forceinline__ void read_pair2(const double2* __restrict__ xe, const
 }
 
 template <int HT, int KIND>
-__global__ void __launch_bounds__(K2_THREADS, 2) k2_link_response(const K2Params p) {
+__global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params p) {
   extern __shared__ double2 smem2[];  // [2 buffers][even, odd][LE] strain tiles, then geo[K2_NGEO][K2_T]
   __shared__ double sky[K2_G][9];     // k, u, v of the block's walkers (Eq. 2.7)
   __shared__ int Kc[K2_G];            // rint of the common 1 AU delay at the block's first sample
