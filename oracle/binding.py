@@ -88,6 +88,7 @@ class Oracle:
         L.orc_spectrum3.argtypes = [C.c_long, _dp, _dp]
         L.orc_loglike.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, C.c_long, C.c_long, _dp, _dp,
                                   _dp]
+        L.orc_fisher.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, C.c_long, C.c_long, _dp]
         L.orc_psd_weights.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, C.c_double,
                                       C.c_int, _dp]
         L.orc_chain.argtypes = (
@@ -217,6 +218,16 @@ class Oracle:
                                   _p(dh), _p(hh))
         assert rc == 0, rc
         return ll, dh, hh
+
+    def fisher(self, tdi, delta, weight, kmin, kmax):
+        """tdi: [D+1][3][N] (walker 0 = centre, walker i = theta + delta_i e_i) -> [D][D]"""
+        tdi, delta, weight = _f64(tdi), _f64(delta), _f64(weight)
+        D = tdi.shape[0] - 1
+        N = tdi.shape[-1]
+        out = np.zeros((D, D))
+        rc = self.lib.orc_fisher(D, N, _p(tdi), _p(delta), _p(weight), kmin, kmax, _p(out))
+        assert rc == 0, rc
+        return out
 
     def psd_weights(self, N, dt, acc_noise, oms_noise, arm_s, generation):
         w = np.zeros((3, N // 2 + 1))

@@ -33,6 +33,8 @@
  *   S4  orc_fft_r2c        : naive DFT, numpy.fft, Parseval (C9)
  *   S5  orc_loglike        : closed forms log L(h=d), log L(lambda d), log L(0) (C10)
  *   orbit / PSD            : arm-length and Kepler invariants, independent numpy forms
+ *   F1  orc_fisher         : linear-model closed form via Parseval (time-domain Gram matrix),
+ *                            symmetry, step independence, Hessian of orc_loglike
  * No function is "parity unpinned".
  */
 #include <math.h>
@@ -670,6 +672,47 @@ int orc_loglike(int B, long N, const double* tdi, const double* data_spec, const
     if (dh) dh[b] = (double)sdh;
     if (hh) hh[b] = (double)shh;
   }
+  free(x);
+  free(spec);
+  return rc;
+}
+
+/* Fisher matrix by first-order finite differences ("The Fisher matrix is computed
+ * from the derivatives of the likelihood function, using first-order finite differences";
+ * reading A19 of DESIGN.md).  Walker 0 is the centre theta, walker i = 1..D is
+ * theta + delta_i e_i.  With the forward difference  d_i h = (h_i - h_0) / delta_i  taken on the
+ * Fourier transforms of the three channels,
+ *   Gamma_ij = (d_i h | d_j h) = sum_c sum_{k=kmin}^{kmax} w_c[k] Re( d_i H_c[k] conj(d_j H_c[k]) ),
+ * the same inner product as Eq. 2.13 (weights of A17).  tdi: [D+1][3][N]; fisher: [D][D]. */
+int orc_fisher(int D, long N, const double* tdi, const double* delta, const double* weight, long kmin,
+               long kmax, double* fisher) {
+  long nf = N / 2 + 1;
+  if (D <= 0 || kmin < 0 || kmin > kmax || kmax > N / 2) return -1;
+  for (int i = 0; i < D; ++i)
+    if (delta[i] == 0.0) return -1;
+  REAL* x = (REAL*)malloc((size_t)N * sizeof(REAL));
+  cplx* spec = (cplx*)malloc((size_t)(D + 1) * 3 * nf * sizeof(cplx));
+  if (!x || !spec) return -3;
+  int rc = 0;
+  for (int b = 0; b <= D && rc == 0; ++b)
+    for (int c = 0; c < 3 && rc == 0; ++c) {
+      for (long n = 0; n < N; ++n) x[n] = (REAL)tdi[((size_t)b * 3 + c) * N + n];
+      rc = fft_r2c_core(N, x, spec + ((size_t)b * 3 + c) * nf);
+    }
+  for (int i = 0; i < D && rc == 0; ++i)
+    for (int j = 0; j < D; ++j) {
+      REAL sum = 0;
+      for (int c = 0; c < 3; ++c)
+        for (long k = kmin; k <= kmax; ++k) {
+          cplx h0 = spec[(size_t)c * nf + k];
+          cplx hi = spec[((size_t)(i + 1) * 3 + c) * nf + k];
+          cplx hj = spec[((size_t)(j + 1) * 3 + c) * nf + k];
+          REAL dire = (hi.re - h0.re) / (REAL)delta[i], diim = (hi.im - h0.im) / (REAL)delta[i];
+          REAL djre = (hj.re - h0.re) / (REAL)delta[j], djim = (hj.im - h0.im) / (REAL)delta[j];
+          sum += (REAL)weight[(size_t)c * nf + k] * (dire * djre + diim * djim);
+        }
+      fisher[(size_t)i * D + j] = (double)sum;
+    }
   free(x);
   free(spec);
   return rc;
