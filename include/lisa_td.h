@@ -132,6 +132,18 @@ LISA_TD_API int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const do
                     const double* data_spec, const double* weight, long long kmin, long long kmax,
                     double* loglike, double* dh, double* hh, void* stream);
 
+/* Fisher matrix by first-order finite differences ("The Fisher matrix is computed
+ * from the derivatives of the likelihood function, using first-order finite differences";
+ * reading A19 of DESIGN.md).  tdi: [D+1][3][N] (A,E,T): walker 0 is the centre theta, walker
+ * i = 1..D is theta + delta_i e_i, all run through S1..S3 by the caller.  With
+ * d_i H = (H_i - H_0)/delta_i on the Fourier transforms,
+ *   fisher[i][j] = (d_i h | d_j h) = sum_c sum_{k=kmin..kmax} w_c[k] Re(d_i H_c[k] conj(d_j H_c[k])).
+ * delta_host: [D] host array, no zero entries.  1 <= D <= 32, D + 1 <= plan capacity.
+ * fisher: [D][D] device, symmetric, written in full.  Deterministic (fixed summation order). */
+LISA_TD_API int lisa_td_fisher(lisa_td_plan* plan, int D, long long N, const double* tdi,
+                   const double* delta_host, const double* weight, long long kmin, long long kmax,
+                   double* fisher, void* stream);
+
 /* Spectrum only (used to build the zero-noise injection): tdi [B][3][N] ->
  * spec [B][3][N/2+1][2]. */
 LISA_TD_API int lisa_td_spectrum(lisa_td_plan* plan, int B, long long N, const double* tdi, double* spec,

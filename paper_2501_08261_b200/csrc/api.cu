@@ -177,6 +177,8 @@ int plan_destroy(Plan*);
 int run_spectrum(Plan*, int, long long, const double*, double*, cudaStream_t);
 int run_loglike(Plan*, int, long long, const double*, const double*, const double*, long long,
                 long long, double*, double*, double*, cudaStream_t);
+int run_fisher(Plan*, int, long long, const double*, const double*, const double*, long long, long long,
+               double*, cudaStream_t);
 extern int g_force_generic;
 
 // ------------------------------------------------------------------ validation helpers
@@ -368,6 +370,17 @@ int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const double* tdi,
   if (rc) return rc;
   REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, data_spec); REQUIRE_PTR(fn, weight); REQUIRE_PTR(fn, loglike);
   return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream);
+}
+
+int lisa_td_fisher(lisa_td_plan* plan, int D, long long N, const double* tdi, const double* delta_host,
+                   const double* weight, long long kmin, long long kmax, double* fisher, void* stream) {
+  const char* fn = "lisa_td_fisher";
+  if (!plan) return set_error(LISA_TD_EINVAL, "%s: plan is NULL", fn);
+  if (!delta_host) return set_error(LISA_TD_EINVAL, "%s: delta_host is NULL", fn);
+  int rc = check_band(fn, N, kmin, kmax);
+  if (rc) return rc;
+  REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, weight); REQUIRE_PTR(fn, fisher);
+  return run_fisher(plan->p, D, N, tdi, delta_host, weight, kmin, kmax, fisher, (cudaStream_t)stream);
 }
 
 int lisa_td_spectrum(lisa_td_plan* plan, int B, long long N, const double* tdi, double* spec, void* stream) {

@@ -19,6 +19,10 @@ namespace lisa {
 
 constexpr int K5_SLICES = 32;
 constexpr int K5_THREADS = 256;
+constexpr int K6_MAXD = 32;     // parameters of the Fisher matrix
+constexpr int K6_TILE = 128;    // (channel, bin) items staged per pass
+constexpr int K6_THREADS = 256;
+constexpr int K6_BLOCKS = 296;  // 2 per SM
 
 struct Plan {
   int B;  // capacity (walkers)
@@ -26,6 +30,7 @@ struct Plan {
   std::map<int, cufftHandle> fft;  // batched D2Z plans keyed by the number of walkers
   double2* spec;     // [B][3][nf]
   double2* partial;  // [B][K5_SLICES]
+  double* fisher_partial;  // [K6_BLOCKS][K6_MAXD * K6_MAXD], allocated on first use
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -92,6 +97,84 @@ __global__ void k5_inner_final(const double2* __restrict__ partial, int B, doubl
   if (hh_out) hh_out[b] = hh;
 }
 
+// ---------------------------------------------------------------- K6: Fisher matrix
+// Gamma_ij = sum_c sum_k w_c[k] Re(d_i H conj d_j H),  d_i H = (H_i - H_0)/delta_i  (PAPER.md:249,
+// reading A19).  The (channel, bin) items of the band are dealt to the blocks in tiles of
+// K6_TILE: the first K6_TILE threads stage the D derivative values and the weight of one item
+// each in shared memory (coalesced reads of the D+1 spectra), then thread = (i, j) pair sums
+// the tile.  Per-block partial matrices are added in a fixed order by k6_fisher_final:
+// deterministic, no atomics.
+struct K6Params {
+  int D;
+  long long nf, kmin, nk;  // nk = kmax - kmin + 1 bins per channel
+  const double2* spec;     // [D+1][3][nf]
+  const double* weight;    // [3][nf]
+  double* partial;         // [gridDim.x][D*D]
+  double inv_delta[K6_MAXD];
+};
+
+__global__ void __launch_bounds__(K6_THREADS) k6_fisher_partial(const K6Params p) {
+  extern __shared__ double2 dsh[];               // [D][K6_TILE]
+  __shared__ double wsh[K6_TILE];
+  const int D = p.D, npairs = D * (D + 1) / 2;
+  const long long items = 3 * p.nk;
+  const long long ntiles = (items + K6_TILE - 1) / K6_TILE;
+  // pairs owned by this thread: p0, p0 + K6_THREADS, ... (at most 3 for D <= 32)
+  double acc[3] = {0.0, 0.0, 0.0};
+  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    __syncthreads();  // previous tile fully consumed
+    if (threadIdx.x < K6_TILE) {
+      const long long it = tile * K6_TILE + threadIdx.x;
+      double w = 0.0;
+      if (it < items) {
+        const int c = (int)(it / p.nk);
+        const long long k = p.kmin + (it - (long long)c * p.nk);
+        w = p.weight[(size_t)c * p.nf + k];
+        const double2 h0 = p.spec[(size_t)c * p.nf + k];
+        for (int i = 0; i < D; ++i) {
+          const double2 hi = p.spec[((size_t)(i + 1) * 3 + c) * p.nf + k];
+          dsh[i * K6_TILE + threadIdx.x] = make_double2((hi.x - h0.x) * p.inv_delta[i], (hi.y - h0.y) * p.inv_delta[i]);
+        }
+      } else {
+        for (int i = 0; i < D; ++i) dsh[i * K6_TILE + threadIdx.x] = make_double2(0.0, 0.0);
+      }
+      wsh[threadIdx.x] = w;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int s = 0; s < 3; ++s) {
+      const int pr = threadIdx.x + s * K6_THREADS;
+      if (pr >= npairs) break;
+      // pair index -> (i, j), i <= j, row-major upper triangle
+      int i = 0, rem = pr;
+      while (rem >= D - i) { rem -= D - i; ++i; }
+      const int j = i + rem;
+      const double2* di = dsh + i * K6_TILE;
+      const double2* dj = dsh + j * K6_TILE;
+      double sum = 0.0;
+      for (int t = 0; t < K6_TILE; ++t) sum = fma(wsh[t], fma(di[t].x, dj[t].x, di[t].y * dj[t].y), sum);
+      acc[s] += sum;
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    const int pr = threadIdx.x + s * K6_THREADS;
+    if (pr < npairs) p.partial[(size_t)blockIdx.x * (K6_MAXD * K6_MAXD) + pr] = acc[s];
+  }
+}
+
+__global__ void k6_fisher_final(const double* __restrict__ partial, int nblocks, int D, double* fisher) {
+  const int pr = blockIdx.x * blockDim.x + threadIdx.x;
+  if (pr >= D * (D + 1) / 2) return;
+  double sum = 0.0;
+  for (int b = 0; b < nblocks; ++b) sum += partial[(size_t)b * (K6_MAXD * K6_MAXD) + pr];
+  int i = 0, rem = pr;
+  while (rem >= D - i) { rem -= D - i; ++i; }
+  const int j = i + rem;
+  fisher[(size_t)i * D + j] = sum;
+  fisher[(size_t)j * D + i] = sum;
+}
+
 static int check_fft(cufftResult r, const char* what) {
   if (r == CUFFT_SUCCESS) return LISA_TD_OK;
   return set_error(LISA_TD_ECUDA, "%s failed: cufftResult %d", what, (int)r);
@@ -123,7 +206,7 @@ int plan_destroy(Plan* pl);
 
 int plan_create(Plan** out, int B, long long N) {
   Plan* pl = new Plan();
-  pl->B = B; pl->N = N; pl->nf = N / 2 + 1; pl->spec = nullptr; pl->partial = nullptr;
+  pl->B = B; pl->N = N; pl->nf = N / 2 + 1; pl->spec = nullptr; pl->partial = nullptr; pl->fisher_partial = nullptr;
   int rc = check_cuda(cudaMalloc(&pl->spec, sizeof(double2) * (size_t)B * 3 * pl->nf), "cudaMalloc(spec)");
   if (rc == LISA_TD_OK) rc = check_cuda(cudaMalloc(&pl->partial, sizeof(double2) * (size_t)B * K5_SLICES), "cudaMalloc(partial)");
   cufftHandle h;
@@ -141,6 +224,7 @@ int plan_destroy(Plan* pl) {
   for (auto& kv : pl->fft) cufftDestroy(kv.second);
   cudaFree(pl->spec);
   cudaFree(pl->partial);
+  cudaFree(pl->fisher_partial);
   delete pl;
   return LISA_TD_OK;
 }
@@ -173,6 +257,36 @@ int run_loglike(Plan* pl, int B, long long N, const double* tdi, const double* d
   LISA_LAUNCH_CHECK("k5_inner_partial");
   k5_inner_final<<<(B + 127) / 128, 128, 0, st>>>(pl->partial, B, loglike, dh, hh);
   LISA_LAUNCH_CHECK("k5_inner_final");
+  return LISA_TD_OK;
+}
+
+// tdi: [D+1][3][N] (walker 0 = centre, walker i = theta + delta_i e_i) -> fisher [D][D]
+int run_fisher(Plan* pl, int D, long long N, const double* tdi, const double* delta_host, const double* weight,
+               long long kmin, long long kmax, double* fisher, cudaStream_t st) {
+  if (N != pl->N) return set_error(LISA_TD_EINVAL, "fisher: N differs from the plan's");
+  if (D < 1 || D > K6_MAXD) return set_error(LISA_TD_EINVAL, "fisher: D must be in [1,%d]", K6_MAXD);
+  if (D + 1 > pl->B) return set_error(LISA_TD_EINVAL, "fisher: D+1=%d walkers exceed the plan's capacity %d", D + 1, pl->B);
+  K6Params p;
+  for (int i = 0; i < K6_MAXD; ++i) p.inv_delta[i] = 0.0;
+  for (int i = 0; i < D; ++i) {
+    if (delta_host[i] == 0.0) return set_error(LISA_TD_EINVAL, "fisher: delta[%d] is zero", i);
+    p.inv_delta[i] = 1.0 / delta_host[i];
+  }
+  if (!pl->fisher_partial)
+    LISA_CUDA(cudaMalloc(&pl->fisher_partial, sizeof(double) * (size_t)K6_BLOCKS * K6_MAXD * K6_MAXD));
+  int rc = run_fft(pl, D + 1, tdi, pl->spec, st);
+  if (rc != LISA_TD_OK) return rc;
+  p.D = D; p.nf = pl->nf; p.kmin = kmin; p.nk = kmax - kmin + 1;
+  p.spec = pl->spec; p.weight = weight; p.partial = pl->fisher_partial;
+  const long long ntiles = (3 * p.nk + K6_TILE - 1) / K6_TILE;
+  const int nblocks = (int)(ntiles < K6_BLOCKS ? ntiles : K6_BLOCKS);
+  const size_t smem = (size_t)D * K6_TILE * sizeof(double2);
+  if (smem > 48 * 1024)
+    LISA_CUDA(cudaFuncSetAttribute(k6_fisher_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k6_fisher_partial<<<nblocks, K6_THREADS, smem, st>>>(p);
+  LISA_LAUNCH_CHECK("k6_fisher_partial");
+  k6_fisher_final<<<(D * (D + 1) / 2 + 127) / 128, 128, 0, st>>>(pl->fisher_partial, nblocks, D, fisher);
+  LISA_LAUNCH_CHECK("k6_fisher_final");
   return LISA_TD_OK;
 }
 

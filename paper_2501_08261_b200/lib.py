@@ -21,7 +21,7 @@ EXPORTS = [
     "lisa_td_last_error", "lisa_td_version", "lisa_td_modes_to_pol", "lisa_td_link_response",
     "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_response_tdi_workspace_bytes",
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
-    "lisa_td_spectrum", "lisa_td_psd_weights", "lisa_td_pipeline_create",
+    "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
     "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_probe_dfma",
     "lisa_td_debug_force_generic",
 ]
@@ -86,6 +86,7 @@ def load() -> C.CDLL:
     L.lisa_td_plan_destroy.argtypes = [vp]
     L.lisa_td_loglike.argtypes = [vp, i32, i64, vp, vp, vp, i64, i64, vp, vp, vp, vp]
     L.lisa_td_spectrum.argtypes = [vp, i32, i64, vp, vp, vp]
+    L.lisa_td_fisher.argtypes = [vp, i32, i64, vp, vp, vp, i64, i64, vp, vp]
     L.lisa_td_psd_weights.argtypes = [i64, dbl, dbl, dbl, dbl, i32, vp]
     L.lisa_td_pipeline_create.argtypes = [C.POINTER(vp), i32, i64, i32, i32]
     L.lisa_td_pipeline_destroy.argtypes = [vp]
@@ -210,6 +211,13 @@ def loglike(plan: Plan, B, N, tdi, data_spec, weight, kmin, kmax, loglike_out, d
 
 def spectrum(plan: Plan, B, N, tdi, spec):
     _check(load().lisa_td_spectrum(plan._h, B, N, _dev(tdi), _dev(spec), _stream()))
+
+
+def fisher(plan: Plan, D, N, tdi, delta, weight, kmin, kmax, fisher_out):
+    delta = np.ascontiguousarray(delta, dtype=np.float64)
+    assert delta.size == D
+    _check(load().lisa_td_fisher(plan._h, D, N, _dev(tdi), _host(delta), _dev(weight), kmin, kmax,
+                                 _dev(fisher_out), _stream()))
 
 
 def psd_weights(N, dt, acc_noise, oms_noise, arm_s, generation) -> np.ndarray:
