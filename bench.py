@@ -289,6 +289,35 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    # ---- batched finite-difference Fisher matrix, D = 15
+    # parameters = 16 walkers (centre + 15 perturbed; the first 16 walkers of the batch, which
+    # are 1e-3 perturbations of walker 0, stand in for them) through S1..S3 + lisa_td_fisher
+    D = 15
+    fis = torch.empty((D, D), dtype=f64, device=device)
+    delta = np.full(D, 1e-3)
+
+    def fisher_step():
+        lib.modes_to_pol(D + 1, N, inp["l"], inp["m"], g("amp"), g("phase"), g("alpha"), g("beta"), g("gamma"),
+                         g("iota"), g("phi"), g("psi"), None, hp, hc)
+        lib.link_response(D + 1, N, t0, dt, ORDER, inp["margin_y"], hp, hc, g("lam"), g("beta_sky"), inp["orbit"], y)
+        lib.tdi2(D + 1, N, t0, dt, ORDER, 20, 1, inp["margin_lo"], inp["margin_hi"], y, inp["orbit"], tdi)
+        lib.fisher(plan, D, N, tdi, delta, weight, kmin, kmax, fis)
+    for _ in range(3):
+        fisher_step()
+    fe = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    torch.cuda.synchronize()
+    fe[0].record()
+    for _ in range(5):
+        fisher_step()
+    fe[1].record()
+    for _ in range(5):
+        lib.fisher(plan, D, N, tdi, delta, weight, kmin, kmax, fis)
+    fe[2].record()
+    torch.cuda.synchronize()
+    fisher_info = {"D": D, "walkers": D + 1, "ms_per_matrix": fe[0].elapsed_time(fe[1]) / 5,
+                   "ms_fft_plus_k6": fe[1].elapsed_time(fe[2]) / 5,
+                   "cite": "PAPER.md:249 (first-order finite differences), DESIGN.md reading A19"}
+
     # ---- roofline of the dominant kernel (S2, link response)
     k2_ms = stage_ms["S2_link_response"]
     ws = B * N
@@ -355,8 +384,9 @@ def run_ours(args):
         "samples_per_s": value * N, "stage_ms": stage_ms, "roofline": roofline, "cpu_baseline": cpu_baseline,
         "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
-            "k5_inner_final": 1, "cufft (library)": "D2Z batch 192"},
+            "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
+        "next": {"fisher": fisher_info},
     }
     print(json.dumps(line))
     plan.close()

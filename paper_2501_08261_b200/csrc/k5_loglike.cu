@@ -5,6 +5,12 @@
 //   (d|h)_b = sum_c sum_{k=kmin..kmax} w_c[k] Re(D_c[k] conj(H_{b,c}[k]))
 //   (h|h)_b = sum_c sum_k w_c[k] |H_{b,c}[k]|^2         log L_b = (d|h)_b - (h|h)_b / 2
 //
+// FFT: the real series x[0..N) is handed to cuFFT as the complex series z[m] = x[2m] + i x[2m+1]
+// of length M = N/2 (one Z2Z pass instead of D2Z's Z2Z + a full-spectrum post-processing pass);
+// the real-input spectrum is recovered only where it is used -- inside the band -- by the
+// textbook split  X[k] = E[k] + e^{-2 pi i k/N} O[k],  E = (Z[k] + conj Z[M-k])/2,
+// O = -i (Z[k] - conj Z[M-k])/2, fused into the reduction kernels (packed_bin below).
+//
 // Reduction: grid (K5_SLICES, B); each block sums a contiguous slice of the band for the three
 // channels of one walker (per-thread partials -> warp shuffles -> one value per warp ->
 // first warp), writes one (dh, hh) pair; a second tiny kernel adds the K5_SLICES pairs of
@@ -28,10 +34,23 @@ struct Plan {
   int B;  // capacity (walkers)
   long long N, nf;
   std::map<int, cufftHandle> fft;  // batched D2Z plans keyed by the number of walkers
-  double2* spec;     // [B][3][nf]
+  double2* spec;     // [B][3][M] packed half-length spectra Z (M = N/2)
   double2* partial;  // [B][K5_SLICES]
   double* fisher_partial;  // [K6_BLOCKS][K6_MAXD * K6_MAXD], allocated on first use
 };
+
+// X[k] of the real series from the packed spectrum Z (row of M = N/2 values), 0 <= k <= M.
+// cs = (cos, sin)(2 pi k / N).
+__device__ __forceinline__ double2 packed_bin(const double2* __restrict__ Z, long long M, long long k, double c, double s) {
+  const double2 a = Z[k == M ? 0 : k];
+  const double2 b = Z[k == 0 ? 0 : M - k];
+  const double er = 0.5 * (a.x + b.x), ei = 0.5 * (a.y - b.y);
+  const double orr = 0.5 * (a.y + b.y), oi = -0.5 * (a.x - b.x);
+  return make_double2(er + fma(c, orr, s * oi), ei + fma(c, oi, -s * orr));
+}
+__device__ __forceinline__ void bin_twiddle(long long k, double two_pi_over_N, double& c, double& s) {
+  sincos_d((double)k * two_pi_over_N, s, c);
+}
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -42,27 +61,25 @@ __device__ __forceinline__ double warp_sum(double v) {
 __global__ void __launch_bounds__(K5_THREADS) k5_inner_partial(
     const double2* __restrict__ spec, const double2* __restrict__ data,
     const double* __restrict__ weight, long long nf, long long kmin, long long kmax,
-    double2* __restrict__ partial) {
+    double two_pi_over_N, double2* __restrict__ partial) {
   const int b = blockIdx.y, slice = blockIdx.x;
   const long long nk = kmax - kmin + 1;
   const long long per = (nk + K5_SLICES - 1) / K5_SLICES;
   const long long k0 = kmin + (long long)slice * per;
   const long long k1 = min(k0 + per, kmax + 1);
+  const long long M = nf - 1;
   double dh = 0.0, hh = 0.0;
+  for (long long k = k0 + threadIdx.x; k < k1; k += K5_THREADS) {
+    double cw, sw;
+    bin_twiddle(k, two_pi_over_N, cw, sw);
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    const double2* H = spec + ((size_t)b * 3 + c) * nf;
-    const double2* D = data + (size_t)c * nf;
-    const double* W = weight + (size_t)c * nf;
-    double dhc = 0.0, hhc = 0.0;
-    for (long long k = k0 + threadIdx.x; k < k1; k += K5_THREADS) {
-      const double2 h = H[k], d = D[k];
-      const double w = W[k];
-      dhc = fma(w, fma(d.x, h.x, d.y * h.y), dhc);
-      hhc = fma(w, fma(h.x, h.x, h.y * h.y), hhc);
+    for (int c = 0; c < 3; ++c) {
+      const double2 h = packed_bin(spec + ((size_t)b * 3 + c) * M, M, k, cw, sw);
+      const double2 d = data[(size_t)c * nf + k];
+      const double w = weight[(size_t)c * nf + k];
+      dh = fma(w, fma(d.x, h.x, d.y * h.y), dh);
+      hh = fma(w, fma(h.x, h.x, h.y * h.y), hh);
     }
-    dh += dhc;
-    hh += hhc;
   }
   __shared__ double sdh[K5_THREADS / 32], shh[K5_THREADS / 32];
   dh = warp_sum(dh);
@@ -107,7 +124,8 @@ __global__ void k5_inner_final(const double2* __restrict__ partial, int B, doubl
 struct K6Params {
   int D;
   long long nf, kmin, nk;  // nk = kmax - kmin + 1 bins per channel
-  const double2* spec;     // [D+1][3][nf]
+  const double2* spec;     // [D+1][3][M] packed
+  double two_pi_over_N;
   const double* weight;    // [3][nf]
   double* partial;         // [gridDim.x][D*D]
   double inv_delta[K6_MAXD];
@@ -130,9 +148,12 @@ __global__ void __launch_bounds__(K6_THREADS) k6_fisher_partial(const K6Params p
         const int c = (int)(it / p.nk);
         const long long k = p.kmin + (it - (long long)c * p.nk);
         w = p.weight[(size_t)c * p.nf + k];
-        const double2 h0 = p.spec[(size_t)c * p.nf + k];
+        const long long M = p.nf - 1;
+        double cw, sw;
+        bin_twiddle(k, p.two_pi_over_N, cw, sw);
+        const double2 h0 = packed_bin(p.spec + (size_t)c * M, M, k, cw, sw);
         for (int i = 0; i < D; ++i) {
-          const double2 hi = p.spec[((size_t)(i + 1) * 3 + c) * p.nf + k];
+          const double2 hi = packed_bin(p.spec + ((size_t)(i + 1) * 3 + c) * M, M, k, cw, sw);
           dsh[i * K6_TILE + threadIdx.x] = make_double2((hi.x - h0.x) * p.inv_delta[i], (hi.y - h0.y) * p.inv_delta[i]);
         }
       } else {
@@ -189,9 +210,9 @@ static int get_fft(Plan* pl, int B, cufftHandle* h) {
   cufftHandle f;
   int rc = check_fft(cufftCreate(&f), "cufftCreate");
   if (rc != LISA_TD_OK) return rc;
-  long long n[1] = {pl->N};
+  long long n[1] = {pl->N / 2};
   size_t ws = 0;
-  rc = check_fft(cufftMakePlanMany64(f, 1, n, nullptr, 1, pl->N, nullptr, 1, pl->nf, CUFFT_D2Z, 3LL * B, &ws),
+  rc = check_fft(cufftMakePlanMany64(f, 1, n, nullptr, 1, pl->N / 2, nullptr, 1, pl->N / 2, CUFFT_Z2Z, 3LL * B, &ws),
                  "cufftMakePlanMany64");
   if (rc != LISA_TD_OK) {
     cufftDestroy(f);
@@ -238,11 +259,30 @@ static int run_fft(Plan* pl, int B, const double* tdi, double2* spec, cudaStream
   if (rc != LISA_TD_OK) return rc;
   rc = check_fft(cufftSetStream(h, st), "cufftSetStream");
   if (rc != LISA_TD_OK) return rc;
-  return check_fft(cufftExecD2Z(h, const_cast<double*>(tdi), reinterpret_cast<cufftDoubleComplex*>(spec)), "cufftExecD2Z");
+  return check_fft(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(const_cast<double*>(tdi)),
+                                reinterpret_cast<cufftDoubleComplex*>(spec), CUFFT_FORWARD),
+                   "cufftExecZ2Z");
 }
+// full real-input spectrum [rows][nf] from the packed spectra [rows][M] (not on the timed path)
+__global__ void k5_unpack_spectrum(const double2* __restrict__ Z, long long rows, long long nf, double two_pi_over_N,
+                                   double2* __restrict__ out) {
+  const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long row = blockIdx.y;
+  if (k >= nf) return;
+  double cw, sw;
+  bin_twiddle(k, two_pi_over_N, cw, sw);
+  out[(size_t)row * nf + k] = packed_bin(Z + (size_t)row * (nf - 1), nf - 1, k, cw, sw);
+}
+
 int run_spectrum(Plan* pl, int B, long long N, const double* tdi, double* spec, cudaStream_t st) {
   if (N != pl->N) return set_error(LISA_TD_EINVAL, "spectrum: N differs from the plan's");
-  return run_fft(pl, B, tdi, reinterpret_cast<double2*>(spec), st);
+  int rc = run_fft(pl, B, tdi, pl->spec, st);
+  if (rc != LISA_TD_OK) return rc;
+  dim3 grid((unsigned)((pl->nf + 255) / 256), (unsigned)(3 * B));
+  k5_unpack_spectrum<<<grid, 256, 0, st>>>(pl->spec, 3LL * B, pl->nf, 6.283185307179586476925 / (double)N,
+                                           reinterpret_cast<double2*>(spec));
+  LISA_LAUNCH_CHECK("k5_unpack_spectrum");
+  return LISA_TD_OK;
 }
 
 int run_loglike(Plan* pl, int B, long long N, const double* tdi, const double* data_spec,
@@ -253,7 +293,7 @@ int run_loglike(Plan* pl, int B, long long N, const double* tdi, const double* d
   if (rc != LISA_TD_OK) return rc;
   dim3 grid(K5_SLICES, (unsigned)B);
   k5_inner_partial<<<grid, K5_THREADS, 0, st>>>(pl->spec, reinterpret_cast<const double2*>(data_spec), weight,
-                                                pl->nf, kmin, kmax, pl->partial);
+                                                pl->nf, kmin, kmax, 6.283185307179586476925 / (double)N, pl->partial);
   LISA_LAUNCH_CHECK("k5_inner_partial");
   k5_inner_final<<<(B + 127) / 128, 128, 0, st>>>(pl->partial, B, loglike, dh, hh);
   LISA_LAUNCH_CHECK("k5_inner_final");
@@ -278,6 +318,7 @@ int run_fisher(Plan* pl, int D, long long N, const double* tdi, const double* de
   if (rc != LISA_TD_OK) return rc;
   p.D = D; p.nf = pl->nf; p.kmin = kmin; p.nk = kmax - kmin + 1;
   p.spec = pl->spec; p.weight = weight; p.partial = pl->fisher_partial;
+  p.two_pi_over_N = 6.283185307179586476925 / (double)N;
   const long long ntiles = (3 * p.nk + K6_TILE - 1) / K6_TILE;
   const int nblocks = (int)(ntiles < K6_BLOCKS ? ntiles : K6_BLOCKS);
   const size_t smem = (size_t)D * K6_TILE * sizeof(double2);
