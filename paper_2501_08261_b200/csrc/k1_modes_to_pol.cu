@@ -214,7 +214,7 @@ __device__ __forceinline__ void k1_load(const double* __restrict__ ptr, size_t n
 }
 
 template <int V>
-__global__ void __launch_bounds__(K1_THREADS) k1_modes_to_pol_std5(const K1FastParams p) {
+__global__ void __launch_bounds__(K1_THREADS, 3) k1_modes_to_pol_std5(const K1FastParams p) {
   __shared__ quat Qc;
   __shared__ double rot[2];
   const int b = blockIdx.y;
