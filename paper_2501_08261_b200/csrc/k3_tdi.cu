@@ -273,7 +273,12 @@ struct K3Geom {
   static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
   static constexpr int CBUF = K3_PAIRS * K3_TS * CS;  // doubles of the stencil staging area
   static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange
-  static constexpr int UNION = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
+  // y buffer 0 is private (its first TMA copy overlaps the coefficient phase); the stencil
+  // staging area shares its space with y buffer 1, which is first filled after phase 1
+  static constexpr int UNION_PRIV = YBUF + (YBUF > CBUF ? YBUF : CBUF);
+  static constexpr int UNION_ALIAS = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
+  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= 227 * 1024;
+  static constexpr int UNION = PRIVATE0 ? UNION_PRIV : UNION_ALIAS;
   static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
 };
 
@@ -287,7 +292,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
   static_assert(CS >= WIN && (CS & 1), "stencil row stride");
   extern __shared__ __align__(128) double smem[];
   double* ys = smem;                    // [2][WC][6][TW]   (phase 2)
-  double* cbuf = smem;                  // [12][32][CS]     (phase 1, aliased)
+  double* cbuf = smem + (G::PRIVATE0 ? G::YBUF : 0);  // [12][32][CS]  (phase 1; aliased with y buffer 1, or with both)
   double* xs = smem + G::UNION;         // [2][3][TS][XS]
   double* Ls = xs + G::XBUF;            // [32][6]
   const int lane = threadIdx.x & 31;
@@ -299,6 +304,35 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
     mbar_init(&mbar[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
+  const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
+  // Walker chunks arrive by TMA: ONE 2-D tiled copy per chunk (box = TW samples x 96 rows of the
+  // [B*6][N] matrix; parts of the box outside the matrix are zero-filled by the hardware, which
+  // covers both the grid edges and a ragged last chunk), completion counted on the buffer's
+  // mbarrier.  The tensor map needs 16-byte row strides, so odd N takes the zero-filling
+  // cp.async path instead.
+  const long long g0 = n0 + LOW - PAD;
+  auto prefetch = [&](int chunk, int buf) {
+    double* dst = ys + (size_t)buf * G::YBUF;
+    if (use_tma) {
+      if (threadIdx.x == 0) {
+        mbar_arrive_expect_tx(&mbar[buf], (unsigned)(G::YBUF * sizeof(double)));
+        tma_load_2d(dst, &tmap, (int)g0, chunk * K3_WC * 6, &mbar[buf]);
+      }
+    } else {
+      const int nrows = min(K3_WC, p.B - chunk * K3_WC) * 6;
+      const double* src0 = p.y + (size_t)chunk * K3_WC * 6 * p.N + g0;
+      for (int row = wid; row < K3_WC * 6; row += NWARPS) {
+        const double* src = src0 + (size_t)row * p.N;
+        for (int i = lane; i < TW; i += 32) {
+          const long long g = g0 + i;
+          const bool ok = row < nrows && g >= 0 && g < p.N;
+          cp_async8_zfill(dst + row * TW + i, ok ? src + i : p.y, ok);
+        }
+      }
+      cp_async_commit();
+    }
+  };
+  if (G::PRIVATE0) prefetch(0, 0);  // chunk 0 lands in y buffer 0 while the coefficients are computed
   // ---- phase 1a: light travel times of the tile's samples
   if (threadIdx.x < K3_TS) {
     double L[6];
@@ -351,36 +385,8 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
   __syncthreads();  // cbuf is dead from here on: its space becomes the y buffers
 
   // ---- phase 2: stream walkers
-  const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
-  // Walker chunks arrive by TMA: ONE 2-D tiled copy per chunk (box = TW samples x 96 rows of the
-  // [B*6][N] matrix; parts of the box outside the matrix are zero-filled by the hardware, which
-  // covers both the grid edges and a ragged last chunk), completion counted on the buffer's
-  // mbarrier.  The tensor map needs 16-byte row strides, so odd N takes the zero-filling
-  // cp.async path instead.
-  const long long g0 = n0 + LOW - PAD;
-  auto prefetch = [&](int chunk, int buf) {
-    double* dst = ys + (size_t)buf * G::YBUF;
-    if (use_tma) {
-      if (threadIdx.x == 0) {
-        mbar_arrive_expect_tx(&mbar[buf], (unsigned)(G::YBUF * sizeof(double)));
-        tma_load_2d(dst, &tmap, (int)g0, chunk * K3_WC * 6, &mbar[buf]);
-      }
-    } else {
-      const int nrows = min(K3_WC, p.B - chunk * K3_WC) * 6;
-      const double* src0 = p.y + (size_t)chunk * K3_WC * 6 * p.N + g0;
-      for (int row = wid; row < K3_WC * 6; row += NWARPS) {
-        const double* src = src0 + (size_t)row * p.N;
-        for (int i = lane; i < TW; i += 32) {
-          const long long g = g0 + i;
-          const bool ok = row < nrows && g >= 0 && g < p.N;
-          cp_async8_zfill(dst + row * TW + i, ok ? src + i : p.y, ok);
-        }
-      }
-      cp_async_commit();
-    }
-  };
-  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // cbuf (generic writes) -> ys (TMA writes)
-  prefetch(0, 0);
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // cbuf (generic writes) -> y buffer 1 (TMA writes)
+  if (!G::PRIVATE0) prefetch(0, 0);
   for (int c = 0; c < n_chunks; ++c) {
     const int buf = c & 1;
     if (c + 1 < n_chunks) prefetch(c + 1, buf ^ 1);
