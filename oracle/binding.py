@@ -88,6 +88,7 @@ class Oracle:
         L.orc_spectrum3.argtypes = [C.c_long, _dp, _dp]
         L.orc_loglike.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, C.c_long, C.c_long, _dp, _dp,
                                   _dp]
+        L.orc_upsample2.argtypes = [C.c_int, C.c_long, _dp, _dp]
         L.orc_fisher.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, C.c_long, C.c_long, _dp]
         L.orc_psd_weights.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, C.c_double,
                                       C.c_int, _dp]
@@ -218,6 +219,16 @@ class Oracle:
                                   _p(dh), _p(hh))
         assert rc == 0, rc
         return ll, dh, hh
+
+    def upsample2(self, coarse):
+        """[B][N/2+1] on the 2 dt grid -> [B][N] on the dt grid (linear interpolation)"""
+        coarse = _f64(coarse)
+        B, Nc = coarse.shape
+        N = 2 * (Nc - 1)
+        out = np.zeros((B, N))
+        rc = self.lib.orc_upsample2(B, N, _p(coarse), _p(out))
+        assert rc == 0, rc
+        return out
 
     def fisher(self, tdi, delta, weight, kmin, kmax):
         """tdi: [D+1][3][N] (walker 0 = centre, walker i = theta + delta_i e_i) -> [D][D]"""

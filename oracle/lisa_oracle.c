@@ -33,6 +33,8 @@
  *   S4  orc_fft_r2c        : naive DFT, numpy.fft, Parseval (C9)
  *   S5  orc_loglike        : closed forms log L(h=d), log L(lambda d), log L(0) (C10)
  *   orbit / PSD            : arm-length and Kepler invariants, independent numpy forms
+ *   UP  orc_upsample2      : exact on linear series, identity on even samples, closed-form
+ *                            midpoint error of a quadratic
  *   F1  orc_fisher         : linear-model closed form via Parseval (time-domain Gram matrix),
  *                            symmetry, step independence, Hessian of orc_loglike
  * No function is "parity unpinned".
@@ -351,6 +353,22 @@ double orc_delay_read(const double* x, long N, long n, double D, int order) {
 }
 
 /* ------------------------------------------------------------------ S2 -- */
+
+/* 10 s -> 5 s (the waveforms are sampled "every Delta t = 10 s and then linearly
+ * interpolate[d] ... to generate the arm and TDI responses with a sampling time of 5 s"; reading
+ * A20 of DESIGN.md).  Coarse series c[0..Nc), Nc = N/2 + 1, on t0 + i (2 dt); fine series on
+ * t0 + n dt:  x[2i] = c[i],  x[2i+1] = (c[i] + c[i+1]) / 2. */
+int orc_upsample2(int B, long N, const double* coarse, double* fine) {
+  if (B <= 0 || N < 2 || (N & 1)) return -1;
+  long Nc = N / 2 + 1;
+  for (int b = 0; b < B; ++b)
+    for (long n = 0; n < N; ++n) {
+      const double* c = coarse + (size_t)b * Nc;
+      REAL v = (n & 1) ? ((REAL)c[n / 2] + (REAL)c[n / 2 + 1]) / 2 : (REAL)c[n / 2];
+      fine[(size_t)b * N + n] = (double)v;
+    }
+  return 0;
+}
 
 static REAL dot3(const REAL* a, const REAL* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
 
