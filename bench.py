@@ -314,6 +314,30 @@ def run_ours(args):
         lib.fisher(plan, D, N, tdi, delta, weight, kmin, kmax, fis)
     fe[2].record()
     torch.cuda.synchronize()
+    # ---- the paper's 10 s -> 5 s trick: S1 on N/2+1 coarse samples
+    # (every other sample of the same inputs) + lisa_td_link_response_up2
+    Nc = N // 2 + 1
+    cz = lambda k: torch.cat([inp[k][..., ::2], inp[k][..., -1:]], dim=-1).contiguous()
+    c_in = {k: cz(k) for k in ("amp", "phase", "alpha", "beta", "gamma")}
+    hpc = torch.empty((B, Nc), dtype=f64, device=device)
+    hcc = torch.empty_like(hpc)
+
+    def up2_step():
+        lib.modes_to_pol(B, Nc, inp["l"], inp["m"], c_in["amp"], c_in["phase"], c_in["alpha"], c_in["beta"],
+                         c_in["gamma"], g("iota"), g("phi"), g("psi"), None, hpc, hcc)
+        lib.link_response_up2(B, N, t0, dt, ORDER, inp["margin_y"], hpc, hcc, g("lam"), g("beta_sky"), inp["orbit"], y)
+    for _ in range(3):
+        up2_step()
+    ue = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ue[0].record()
+    for _ in range(5):
+        up2_step()
+    ue[1].record()
+    torch.cuda.synchronize()
+    up2_info = {"ms_s1_coarse_plus_s2_up2": ue[0].elapsed_time(ue[1]) / 5,
+                "ms_s1_plus_s2_full_rate": stage_ms["S1_modes_to_pol"] + stage_ms["S2_link_response"],
+                "cite": "PAPER.md:243 (10 s sampling, linear interpolation), DESIGN.md reading A20"}
+    del c_in, hpc, hcc
     fisher_info = {"D": D, "walkers": D + 1, "ms_per_matrix": fe[0].elapsed_time(fe[1]) / 5,
                    "ms_fft_plus_k6": fe[1].elapsed_time(fe[2]) / 5,
                    "cite": "PAPER.md:249 (first-order finite differences), DESIGN.md reading A19"}
@@ -386,7 +410,7 @@ def run_ours(args):
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
-        "next": {"fisher": fisher_info},
+        "next": {"fisher": fisher_info, "up2": up2_info},
     }
     print(json.dumps(line))
     plan.close()

@@ -93,6 +93,18 @@ LISA_TD_API int lisa_td_link_response(int B, long long N, double t0, double dt, 
                           const double* beta_sky, const lisa_td_orbit* orbit_host, double* y,
                           void* stream);
 
+/* S2 with the paper's 10 s -> 5 s trick (the waveforms are sampled "every
+ * Delta t = 10 s and then linearly interpolate[d] ... to generate the arm and TDI responses with
+ * a sampling time of 5 s"; reading A20 of DESIGN.md).  hplus_c, hcross_c: [B][N/2+1] on the grid
+ * t0 + i (2 dt) (e.g. lisa_td_modes_to_pol run on N/2+1 samples of the coarse modes); the strain
+ * on the dt grid is x[2i] = c[i], x[2i+1] = (c[i] + c[i+1])/2, formed while the tile is staged
+ * (never materialised).  N must be even; everything else as lisa_td_link_response.  Note the
+ * row stride N/2+1: rows need not be 16-byte aligned, only the base pointers. */
+LISA_TD_API int lisa_td_link_response_up2(int B, long long N, double t0, double dt, int order,
+                              long long margin_y, const double* hplus_c, const double* hcross_c,
+                              const double* lambda, const double* beta_sky,
+                              const lisa_td_orbit* orbit_host, double* y, void* stream);
+
 /* A12 -- link-level common laser noise y_l[n] = p(n - L_l(t_n)/dt) - p[n] (zero outside
  * [margin, N - margin)); p: [N], y: [6][N].  Used to check TDI laser-noise suppression. */
 LISA_TD_API int lisa_td_laser_links(long long N, double t0, double dt, int order, long long margin,

@@ -166,7 +166,7 @@ int run_modes_to_pol(int, long long, int, const int*, const int*, const double*,
                      const double*, const double*, const double*, const double*, const double*,
                      const double*, const double*, double*, double*, cudaStream_t);
 int run_link_response(int, long long, double, double, int, long long, const double*, const double*,
-                      const double*, const double*, const OrbitDev&, double*, cudaStream_t);
+                      const double*, const double*, const OrbitDev&, double*, cudaStream_t, int up2 = 0);
 int run_laser_links(long long, double, double, int, long long, const double*, const OrbitDev&,
                     double*, cudaStream_t);
 int run_tdi(int, long long, double, double, int, int, int, long long, long long, const double*,
@@ -270,6 +270,23 @@ int lisa_td_link_response(int B, long long N, double t0, double dt, int order, l
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
   return run_link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lambda, beta_sky, od, y,
                            (cudaStream_t)stream);
+}
+
+int lisa_td_link_response_up2(int B, long long N, double t0, double dt, int order, long long margin_y,
+                              const double* hplus_c, const double* hcross_c, const double* lambda,
+                              const double* beta_sky, const lisa_td_orbit* orbit_host, double* y,
+                              void* stream) {
+  const char* fn = "lisa_td_link_response_up2";
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (N & 1) return set_error(LISA_TD_EINVAL, "%s: N must be even (got %lld)", fn, N);
+  REQUIRE_PTR(fn, hplus_c); REQUIRE_PTR(fn, hcross_c); REQUIRE_PTR(fn, lambda); REQUIRE_PTR(fn, beta_sky);
+  REQUIRE_PTR(fn, y);
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
+  return run_link_response(B, N, t0, dt, order, margin_y, hplus_c, hcross_c, lambda, beta_sky, od, y,
+                           (cudaStream_t)stream, 1);
 }
 
 int lisa_td_laser_links(long long N, double t0, double dt, int order, long long margin,

@@ -31,6 +31,7 @@ struct K2Params {
   int margin;  // margin_y
   int group;   // walkers per block
   int halo;    // tile halo in samples (bound on |D - Kc| + half + slack)
+  int up2;     // 1: hplus/hcross are [B][N/2+1] on the 2 dt grid, linearly interpolated while staging (A20)
   const double* hplus;
   const double* hcross;
   const double* lambda;
@@ -101,10 +102,28 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
   __syncthreads();
 
   auto prefetch = [&](int w, int buf) {
-    const double* hp = p.hplus + (size_t)(w0 + w) * p.N;
-    const double* hc = p.hcross + (size_t)(w0 + w) * p.N;
     double2* dst = smem2 + (size_t)buf * 2 * LE;
     const long long g0 = n0 - Kc[w] - p.halo;
+    if (p.up2) {
+      // strain sampled every 2 dt, linearly interpolated to the dt grid
+      const long long Nc = p.N / 2 + 1;
+      const double* hp = p.hplus + (size_t)(w0 + w) * Nc;
+      const double* hc = p.hcross + (size_t)(w0 + w) * Nc;
+      for (int i = threadIdx.x; i < tile_len; i += K2_THREADS) {
+        const long long g = g0 + i;
+        double2 v = make_double2(0.0, 0.0);
+        if (g >= 0 && g < p.N) {
+          const long long c = g >> 1;
+          v = make_double2(hp[c], hc[c]);
+          if (g & 1) v = make_double2((v.x + hp[c + 1]) * 0.5, (v.y + hc[c + 1]) * 0.5);
+        }
+        dst[(i & 1) * LE + (i >> 1)] = v;
+      }
+      asm volatile("cp.async.commit_group;\n" ::);  // keeps the group count of the cp.async path
+      return;
+    }
+    const double* hp = p.hplus + (size_t)(w0 + w) * p.N;
+    const double* hc = p.hcross + (size_t)(w0 + w) * p.N;
     for (int i = threadIdx.x; i < tile_len; i += K2_THREADS) {
       const long long g = g0 + i;
       const bool ok = g >= 0 && g < p.N;
@@ -298,8 +317,9 @@ int g_force_generic = 0;  // debug switch (lisa_td_debug_force_generic)
 
 int run_link_response(int B, long long N, double t0, double dt, int order, long long margin_y,
                       const double* hplus, const double* hcross, const double* lambda,
-                      const double* beta_sky, const OrbitDev& orb, double* y, cudaStream_t st) {
+                      const double* beta_sky, const OrbitDev& orb, double* y, cudaStream_t st, int up2) {
   K2Params p;
+  p.up2 = up2;
   p.B = B; p.N = N; p.t0 = t0; p.dt = dt; p.inv_dt = 1.0 / dt;
   p.half = (order + 1) / 2; p.margin = (int)margin_y;
   p.hplus = hplus; p.hcross = hcross; p.lambda = lambda; p.beta_sky = beta_sky; p.y = y;

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "liblisa_td.so")
 
 EXPORTS = [
     "lisa_td_last_error", "lisa_td_version", "lisa_td_modes_to_pol", "lisa_td_link_response",
+    "lisa_td_link_response_up2",
     "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_response_tdi_workspace_bytes",
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
@@ -75,6 +76,7 @@ def load() -> C.CDLL:
     L.lisa_td_modes_to_pol.argtypes = [i32, i64, i32, C.POINTER(i32), C.POINTER(i32)] + [vp] * 11 + [vp]
     L.lisa_td_link_response.argtypes = [i32, i64, dbl, dbl, i32, i64, vp, vp, vp, vp,
                                         C.POINTER(Orbit), vp, vp]
+    L.lisa_td_link_response_up2.argtypes = L.lisa_td_link_response.argtypes
     L.lisa_td_laser_links.argtypes = [i64, dbl, dbl, i32, i64, vp, C.POINTER(Orbit), vp, vp]
     L.lisa_td_tdi2.argtypes = [i32, i64, dbl, dbl, i32, i32, i32, i64, i64, vp, C.POINTER(Orbit),
                                vp, vp]
@@ -158,6 +160,12 @@ def link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lam, beta_sky, o
     o = make_orbit(orbit)
     _check(load().lisa_td_link_response(B, N, t0, dt, order, margin_y, _dev(hplus), _dev(hcross),
                                         _dev(lam), _dev(beta_sky), C.byref(o), _dev(y), _stream()))
+
+
+def link_response_up2(B, N, t0, dt, order, margin_y, hplus_c, hcross_c, lam, beta_sky, orbit, y):
+    o = make_orbit(orbit)
+    _check(load().lisa_td_link_response_up2(B, N, t0, dt, order, margin_y, _dev(hplus_c), _dev(hcross_c),
+                                            _dev(lam), _dev(beta_sky), C.byref(o), _dev(y), _stream()))
 
 
 def laser_links(N, t0, dt, order, margin, p, orbit, y):
