@@ -277,7 +277,7 @@ struct K3Geom {
   // staging area shares its space with y buffer 1, which is first filled after phase 1
   static constexpr int UNION_PRIV = YBUF + (YBUF > CBUF ? YBUF : CBUF);
   static constexpr int UNION_ALIAS = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
-  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= 227 * 1024;
+  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= (K3_TS == 16 ? 112 : 227) * 1024;
   static constexpr int UNION = PRIVATE0 ? UNION_PRIV : UNION_ALIAS;
   static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
 };
