@@ -27,6 +27,11 @@ class OrcOrbit(C.Structure):
         ("t_ref", C.c_double),
         ("r_static", (C.c_double * 3) * 3),
         ("L_static", C.c_double * 6),
+        ("n_tab", C.c_int),
+        ("tab_order", C.c_int),
+        ("t_tab0", C.c_double),
+        ("dt_tab", C.c_double),
+        ("r_tab", C.POINTER(C.c_double)),
     ]
 
 
@@ -47,6 +52,15 @@ def make_orbit(d: dict) -> OrcOrbit:
         o.year_s = float(d["year_s"])
         o.phase0 = float(d.get("phase0", 0.0))
         o.t_ref = float(d.get("t_ref", 0.0))
+    elif d["kind"] == "table":
+        o.kind = 2
+        tab = np.ascontiguousarray(d["r_tab"], dtype=np.float64)
+        assert tab.ndim == 3 and tab.shape[1:] == (3, 3)
+        o._keep = tab  # keep the array alive as long as the struct
+        o.n_tab, o.tab_order = tab.shape[0], int(d.get("tab_order", 7))
+        assert o.tab_order % 2 == 1 and o.n_tab > o.tab_order
+        o.t_tab0, o.dt_tab = float(d["t_tab0"]), float(d["dt_tab"])
+        o.r_tab = tab.ctypes.data_as(C.POINTER(C.c_double))
     else:
         raise ValueError(d["kind"])
     return o

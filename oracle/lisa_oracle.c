@@ -33,6 +33,7 @@
  *   S4  orc_fft_r2c        : naive DFT, numpy.fft, Parseval (C9)
  *   S5  orc_loglike        : closed forms log L(h=d), log L(lambda d), log L(0) (C10)
  *   orbit / PSD            : arm-length and Kepler invariants, independent numpy forms
+ *   orbit TABLE (A21)      : exact on polynomial trajectories, KEPLER1 table vs KEPLER1 closed form
  *   UP  orc_upsample2      : exact on linear series, identity on even samples, closed-form
  *                            midpoint error of a quadratic
  *   F1  orc_fisher         : linear-model closed form via Parseval (time-domain Gram matrix),
@@ -76,10 +77,14 @@ static cplx c_expi(REAL x) { return c_make(cos(x), sin(x)); }
 
 /* Orbit description.  Declared independently of include/lisa_td.h on purpose. */
 typedef struct {
-  int kind; /* 0 = STATIC, 1 = KEPLER1 (reading A8) */
+  int kind; /* 0 = STATIC, 1 = KEPLER1 (reading A8), 2 = TABLE (reading A21) */
   double L_m, a_m, year_s, phase0, t_ref;
   double r_static[3][3]; /* metres, [spacecraft][xyz] */
   double L_static[6];    /* seconds, link order [1,2,3,-1,-2,-3] */
+  /* TABLE: positions tabulated at t_tab0 + j dt_tab, j = 0..n_tab-1 */
+  int n_tab, tab_order;  /* tab_order odd: tab_order + 1 interpolation nodes */
+  double t_tab0, dt_tab;
+  const double* r_tab;   /* [n_tab][3][3] metres */
 } orc_orbit;
 
 /* Link order l = [1,2,3,-1,-2,-3]; (sender, receiver) spacecraft, 1-based
@@ -271,6 +276,34 @@ static void orbit_eval(const orc_orbit* o, REAL t, REAL r[3][3], REAL L[6]) {
     for (int i = 0; i < 3; ++i)
       for (int j = 0; j < 3; ++j) r[i][j] = (REAL)o->r_static[i][j];
     for (int k = 0; k < 6; ++k) L[k] = (REAL)o->L_static[k];
+    return;
+  }
+  if (o->kind == 2) {
+    /* TABLE (orbits "tracked over the whole observation period", ESA-style file;
+     * reading A21): Lagrange interpolation of degree q = tab_order on the q+1 nodes
+     * j0 .. j0+q,  j0 = floor(u) - (q-1)/2 clamped to [0, n_tab-q-1],  u = (t - t_tab0)/dt_tab;
+     * light travel times L_l = |r_r - r_s| / c as for KEPLER1. */
+    int q = o->tab_order;
+    REAL u = (t - (REAL)o->t_tab0) / (REAL)o->dt_tab;
+    long j0 = (long)floor(u) - (q - 1) / 2;
+    if (j0 < 0) j0 = 0;
+    if (j0 > o->n_tab - q - 1) j0 = o->n_tab - q - 1;
+    REAL x = u - (REAL)j0;
+    for (int k = 0; k < 3; ++k)
+      for (int j = 0; j < 3; ++j) r[k][j] = 0;
+    for (int i = 0; i <= q; ++i) {
+      REAL c = 1;
+      for (int m = 0; m <= q; ++m)
+        if (m != i) c *= (x - (REAL)m) / (REAL)(i - m);
+      for (int k = 0; k < 3; ++k)
+        for (int j = 0; j < 3; ++j) r[k][j] += c * (REAL)o->r_tab[((size_t)(j0 + i) * 3 + k) * 3 + j];
+    }
+    for (int k = 0; k < 6; ++k) {
+      const REAL* rs = r[LINK_S[k] - 1];
+      const REAL* rr = r[LINK_R[k] - 1];
+      REAL d0 = rr[0] - rs[0], d1 = rr[1] - rs[1], d2 = rr[2] - rs[2];
+      L[k] = sqrt(d0 * d0 + d1 * d1 + d2 * d2) / ORC_C_LIGHT;
+    }
     return;
   }
   REAL a = (REAL)o->a_m;
