@@ -60,13 +60,28 @@ LISA_TD_API int lisa_td_version(void);
  * kind 0 = STATIC : spacecraft positions r_static[spacecraft][xyz] in metres and the six light
  *                   travel times L_static (seconds, link order) are constants.
  * kind 1 = KEPLER1: reading A8 of DESIGN.md (analytic orbits, first-order solution of Kepler's
- *                   equation, breathing unequal arms; L_l(t) = |r_r(t) - r_s(t)|/c). */
+ *                   equation, breathing unequal arms; L_l(t) = |r_r(t) - r_s(t)|/c).
+ * kind 2 = TABLE  : reading A21 (orbits "tracked over the whole observation period",
+ *                   e.g. an ESA orbit file): spacecraft positions tabulated on a uniform time
+ *                   grid, held in a lisa_td_orbit_table; per sample they are interpolated with a
+ *                   Lagrange polynomial of odd degree q on the q+1 nodes j0..j0+q,
+ *                   j0 = floor((t - t_tab0)/dt_tab) - (q-1)/2 clamped to the table;
+ *                   L_l(t) = |r_r(t) - r_s(t)|/c.  The table must cover [t0, t0 + N dt]. */
+typedef struct lisa_td_orbit_table lisa_td_orbit_table;
 typedef struct {
   int kind;
   double L_m, a_m, year_s, phase0, t_ref;
   double r_static[3][3];
   double L_static[6];
+  const lisa_td_orbit_table* table; /* kind 2 only */
 } lisa_td_orbit;
+
+/* Owns a device copy of the table (the only device memory the library holds besides plans).
+ * r_host: [n_tab][3][3] = [node][spacecraft][xyz] in metres at t_tab0 + j dt_tab; interp_order q
+ * odd in [1,15], n_tab > q.  create synchronises (one host-to-device copy). */
+LISA_TD_API int lisa_td_orbit_table_create(lisa_td_orbit_table** out, int n_tab, double t_tab0, double dt_tab,
+                               int interp_order, const double* r_host);
+LISA_TD_API int lisa_td_orbit_table_destroy(lisa_td_orbit_table* table);
 
 /* S1 -- Eq. 2.4-2.6 (single-sum form; readings A1-A6).
  *   h+ - i hx = e^{2 i psi} sum_k [ h_k frakD^l_{m,2}(R) + (-1)^l conj(h_k) frakD^l_{-m,2}(R) ] sqrt((2l+1)/4pi)

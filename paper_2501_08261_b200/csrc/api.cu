@@ -92,10 +92,42 @@ static void kepler1_host(const lisa_td_orbit* o, long double t, long double r[3]
   }
 }
 
+}  // namespace lisa
+
+// Tabulated orbit: device copy for the kernels, host-side bounds for the margin / halo checks.
+struct lisa_td_orbit_table {
+  int n_tab, order;
+  double t_tab0, dt_tab;
+  double* dev;
+  double max_r, max_L, max_off, max_rate;  // metres, metres, metres, metres per second
+};
+
+namespace lisa {
+
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
   if (!o) return set_error(LISA_TD_EINVAL, "orbit_host is NULL");
   memset(d, 0, sizeof(*d));
   d->kind = o->kind;
+  if (o->kind == 2) {
+    const lisa_td_orbit_table* t = o->table;
+    if (!t) return set_error(LISA_TD_EINVAL, "orbit: kind TABLE needs a lisa_td_orbit_table");
+    d->tab = t->dev;
+    d->n_tab = t->n_tab;
+    d->tab_order = t->order;
+    d->t_tab0 = t->t_tab0;
+    d->inv_dt_tab = 1.0 / t->dt_tab;
+    for (int i = 0; i <= t->order; ++i) {
+      long double den = 1.0L;
+      for (int m = 0; m <= t->order; ++m)
+        if (m != i) den *= (long double)(i - m);
+      d->tab_w[i] = (double)(1.0L / den);
+    }
+    d->max_r_over_c = t->max_r * 1.01 / C_LIGHT;
+    d->max_L = t->max_L * 1.01 / C_LIGHT;
+    d->max_off_over_c = t->max_off * 1.01 / C_LIGHT;
+    d->max_dc_rate = t->max_rate * 1.05 / C_LIGHT;
+    return LISA_TD_OK;
+  }
   if (o->kind == 0) {
     double mr = 0.0, mL = 0.0;
     for (int k = 0; k < 3; ++k) {
@@ -113,6 +145,7 @@ int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
     }
     d->max_r_over_c = mr / C_LIGHT;
     d->max_off_over_c = mr / C_LIGHT;
+    d->max_dc_rate = 0.0;
     d->max_L = mL;
     return LISA_TD_OK;
   }
@@ -158,6 +191,7 @@ int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
   d->max_r_over_c = (double)(mr * 1.001L / C_LIGHT);
   d->max_L = (double)(mL * 1.001L / C_LIGHT);
   d->max_off_over_c = (double)(mo * 1.001L / C_LIGHT);
+  d->max_dc_rate = d->a_over_c * d->w;
   return LISA_TD_OK;
 }
 
@@ -223,6 +257,16 @@ static int check_margin_tdi(const char* fn, long long N, double dt, int order, i
   return LISA_TD_OK;
 }
 
+static int check_table_range(const char* fn, const lisa_td_orbit* o, long long N, double t0, double dt) {
+  if (!o || o->kind != 2 || !o->table) return LISA_TD_OK;
+  const lisa_td_orbit_table* t = o->table;
+  const double t_end = t->t_tab0 + (t->n_tab - 1) * t->dt_tab;
+  if (t0 < t->t_tab0 || t0 + (double)N * dt > t_end)
+    return set_error(LISA_TD_EINVAL, "%s: the orbit table [%g, %g] s does not cover the grid [%g, %g] s", fn,
+                     t->t_tab0, t_end, t0, t0 + (double)N * dt);
+  return LISA_TD_OK;
+}
+
 }  // namespace lisa
 
 using namespace lisa;
@@ -231,6 +275,52 @@ using namespace lisa;
 extern "C" {
 
 const char* lisa_td_last_error(void) { return g_err; }
+
+int lisa_td_orbit_table_create(lisa_td_orbit_table** out, int n_tab, double t_tab0, double dt_tab,
+                               int interp_order, const double* r_host) {
+  const char* fn = "lisa_td_orbit_table_create";
+  if (!out || !r_host) return set_error(LISA_TD_EINVAL, "%s: NULL argument", fn);
+  if (interp_order < 1 || interp_order > 15 || !(interp_order & 1))
+    return set_error(LISA_TD_EINVAL, "%s: interp_order must be odd in [1,15] (got %d)", fn, interp_order);
+  if (n_tab <= interp_order) return set_error(LISA_TD_EINVAL, "%s: n_tab must exceed interp_order", fn);
+  if (!(dt_tab > 0)) return set_error(LISA_TD_EINVAL, "%s: dt_tab must be > 0", fn);
+  lisa_td_orbit_table* t = new lisa_td_orbit_table();
+  t->n_tab = n_tab; t->order = interp_order; t->t_tab0 = t_tab0; t->dt_tab = dt_tab; t->dev = nullptr;
+  t->max_r = t->max_L = t->max_off = t->max_rate = 0.0;
+  double prev_c[3] = {0, 0, 0};
+  for (int j = 0; j < n_tab; ++j) {
+    const double* r = r_host + (size_t)j * 9;
+    double c[3];
+    for (int x = 0; x < 3; ++x) c[x] = (r[x] + r[3 + x] + r[6 + x]) / 3.0;
+    for (int k = 0; k < 3; ++k) {
+      const double* a = r + 3 * k;
+      const double* b = r + 3 * ((k + 1) % 3);
+      t->max_r = fmax(t->max_r, sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]));
+      t->max_L = fmax(t->max_L, sqrt((a[0] - b[0]) * (a[0] - b[0]) + (a[1] - b[1]) * (a[1] - b[1]) + (a[2] - b[2]) * (a[2] - b[2])));
+      t->max_off = fmax(t->max_off, sqrt((a[0] - c[0]) * (a[0] - c[0]) + (a[1] - c[1]) * (a[1] - c[1]) + (a[2] - c[2]) * (a[2] - c[2])));
+    }
+    if (j > 0)
+      t->max_rate = fmax(t->max_rate, sqrt((c[0] - prev_c[0]) * (c[0] - prev_c[0]) + (c[1] - prev_c[1]) * (c[1] - prev_c[1]) +
+                                           (c[2] - prev_c[2]) * (c[2] - prev_c[2])) / dt_tab);
+    for (int x = 0; x < 3; ++x) prev_c[x] = c[x];
+  }
+  int rc = check_cuda(cudaMalloc(&t->dev, sizeof(double) * 9 * (size_t)n_tab), "cudaMalloc(orbit table)");
+  if (rc == LISA_TD_OK)
+    rc = check_cuda(cudaMemcpy(t->dev, r_host, sizeof(double) * 9 * (size_t)n_tab, cudaMemcpyHostToDevice), "cudaMemcpy(orbit table)");
+  if (rc != LISA_TD_OK) {
+    cudaFree(t->dev);
+    delete t;
+    return rc;
+  }
+  *out = t;
+  return LISA_TD_OK;
+}
+int lisa_td_orbit_table_destroy(lisa_td_orbit_table* t) {
+  if (!t) return LISA_TD_OK;
+  cudaFree(t->dev);
+  delete t;
+  return LISA_TD_OK;
+}
 int lisa_td_version(void) { return 100; }
 void lisa_td_debug_force_generic(int on) { g_force_generic = on; }
 
@@ -267,6 +357,7 @@ int lisa_td_link_response(int B, long long N, double t0, double dt, int order, l
   REQUIRE_PTR(fn, y);
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
   return run_link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lambda, beta_sky, od, y,
                            (cudaStream_t)stream);
@@ -284,6 +375,7 @@ int lisa_td_link_response_up2(int B, long long N, double t0, double dt, int orde
   REQUIRE_PTR(fn, y);
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
   return run_link_response(B, N, t0, dt, order, margin_y, hplus_c, hcross_c, lambda, beta_sky, od, y,
                            (cudaStream_t)stream, 1);
@@ -297,6 +389,7 @@ int lisa_td_laser_links(long long N, double t0, double dt, int order, long long 
   REQUIRE_PTR(fn, p); REQUIRE_PTR(fn, y);
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   const long long need = (long long)ceil(od.max_L / dt) + (order + 1) / 2;
   if (margin < need || N < 2 * margin)
     return set_error(LISA_TD_EINVAL, "%s: margin=%lld must be >= %lld and N >= 2*margin", fn, margin, need);
@@ -313,6 +406,7 @@ int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int genera
   REQUIRE_PTR(fn, y); REQUIRE_PTR(fn, tdi);
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
   return run_tdi(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi,
                  (cudaStream_t)stream);
@@ -339,6 +433,7 @@ int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, lo
                      workspace_bytes, lisa_td_response_tdi_workspace_bytes(B, N));
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
   if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
   double* y = static_cast<double*>(workspace);
@@ -531,6 +626,7 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
   if ((rc = check_band(fn, N, kmin, kmax))) return rc;
   OrbitDev od;
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
   if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
 

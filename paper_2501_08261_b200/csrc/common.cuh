@@ -67,7 +67,13 @@ struct OrbitDev {
   double L[6];                    // STATIC light travel times [s]
   double max_r_over_c;            // host-side bounds used for margin validation [s]
   double max_L;                   // [s]
-  double max_off_over_c;          // max |r_k - a(cos M, sin M, 0)| / c (STATIC: max |r_k| / c) [s]
+  double max_off_over_c;          // max |r_k - common part| / c (STATIC: max |r_k| / c) [s]
+  double max_dc_rate;             // max |d/dt (common part)| / c: drift of the common delay [s/s]
+  // TABLE (reading A21): positions tabulated at t_tab0 + j dt_tab, Lagrange degree tab_order
+  const double* tab;              // DEVICE [n_tab][3][3] metres (owned by a lisa_td_orbit_table)
+  int n_tab, tab_order;
+  double t_tab0, inv_dt_tab;
+  double tab_w[16];               // 1 / prod_{m != i} (i - m), i = 0..tab_order
 };
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* out);
 
@@ -118,21 +124,63 @@ __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
 }
 
 // ------------------------------------------------------------------ orbit evaluation
-// delta[k][xyz]: spacecraft positions minus the common part a(cM, sM, 0)  (STATIC: the
-// positions themselves, cM = sM = 0).
+// TABLE: Lagrange interpolation of degree q on the nodes j0..j0+q, j0 = floor(u) - (q-1)/2
+// clamped to the table, u = (t - t_tab0)/dt_tab (reading A21); the common part is the centroid.
+__device__ __forceinline__ void orbit_table_eval(const OrbitDev& o, double t, double (&d)[3][3], double (&rc_s)[3]) {
+  const int q = o.tab_order;
+  const double u = (t - o.t_tab0) * o.inv_dt_tab;
+  int j0 = (int)floor(u) - (q - 1) / 2;
+  j0 = max(0, min(j0, o.n_tab - q - 1));
+  const double x = u - (double)j0;
+  double r[3][3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) r[k][j] = 0.0;
+#pragma unroll 1
+  for (int i = 0; i <= q; ++i) {
+    double c = o.tab_w[i];
+#pragma unroll 1
+    for (int m = 0; m <= q; ++m)
+      if (m != i) c *= x - (double)m;
+    const double* row = o.tab + (size_t)(j0 + i) * 9;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) r[k][j] = fma(c, __ldg(row + 3 * k + j), r[k][j]);
+  }
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    const double c = (r[0][j] + r[1][j] + r[2][j]) * (1.0 / 3.0);
+    rc_s[j] = c / C_LIGHT;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) d[k][j] = r[k][j] - c;
+  }
+}
+
+// d[k][xyz]: spacecraft positions minus a common part; rc_s: that common part as a light
+// travel time [s] per unit direction.  KEPLER1: common part a(cos M, sin M, 0); STATIC: zero
+// (d = the positions themselves); TABLE: the centroid.
 __device__ __forceinline__ void orbit_offsets(const OrbitDev& o, double t, double (&d)[3][3],
-                                              double& cM, double& sM) {
+                                              double (&rc_s)[3]) {
   if (o.kind == 0) {
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
       for (int j = 0; j < 3; ++j) d[k][j] = o.r[k][j];
-    cM = 0.0;
-    sM = 0.0;
+    rc_s[0] = rc_s[1] = rc_s[2] = 0.0;
     return;
   }
+  if (o.kind == 2) {
+    orbit_table_eval(o, t, d, rc_s);
+    return;
+  }
+  double cM, sM;
   double M = fma(o.w, t - o.t_ref, -o.phase0);
   sincos_d(M, sM, cM);
+  rc_s[0] = o.a_over_c * cM;
+  rc_s[1] = o.a_over_c * sM;
+  rc_s[2] = 0.0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     // M_k = M - sigma_k
@@ -160,8 +208,8 @@ __device__ __forceinline__ void orbit_arm_times(const OrbitDev& o, double t, dou
     for (int l = 0; l < 6; ++l) L[l] = o.L[l];
     return;
   }
-  double d[3][3], cM, sM;
-  orbit_offsets(o, t, d, cM, sM);
+  double d[3][3], rc_s[3];
+  orbit_offsets(o, t, d, rc_s);
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
     const int s = (l + 2) % 3, r = (l + 1) % 3;  // link l+1: sender, receiver

@@ -21,7 +21,7 @@ namespace lisa {
 constexpr int K2_T = 256;        // output samples per block
 constexpr int K2_THREADS = 128;  // two adjacent samples per thread
 constexpr int K2_G = 16;         // walkers per block (upper bound)
-constexpr int K2_NGEO = 20;      // geometry fields per sample
+constexpr int K2_NGEO = 21;      // geometry fields per sample
 
 struct K2Params {
   int B;
@@ -96,6 +96,10 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
       double sM, cM;
       sincos_d(fma(p.orb.w, fma((double)n0, p.dt, p.t0) - p.orb.t_ref, -p.orb.phase0), sM, cM);
       Dc0 = p.orb.a_over_c * p.inv_dt * fma(s[0], cM, s[1] * sM);
+    } else if (KIND == 2) {
+      double d0[3][3], rc0[3];
+      orbit_offsets(p.orb, fma((double)n0, p.dt, p.t0), d0, rc0);
+      Dc0 = p.inv_dt * fma(s[0], rc0[0], fma(s[1], rc0[1], s[2] * rc0[2]));
     }
     Kc[threadIdx.x] = __double2int_rn(Dc0);
   }
@@ -141,11 +145,12 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 #pragma unroll 1
   for (int c = 0; c < 2; ++c) {
     double* gq = geo + 2 * threadIdx.x + c;
-    double d[3][3], cM, sM;
-    orbit_offsets(p.orb, fma((double)(na + c), p.dt, p.t0), d, cM, sM);
+    double d[3][3], rc_s[3];
+    orbit_offsets(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s);
     const double sc = p.inv_dt / C_LIGHT;
-    gq[0 * K2_T] = p.orb.a_over_c * p.inv_dt * cM;   // common 1 AU delay per unit k (samples)
-    gq[1 * K2_T] = p.orb.a_over_c * p.inv_dt * sM;
+    gq[0 * K2_T] = rc_s[0] * p.inv_dt;   // common (1 AU) delay per unit k (samples)
+    gq[1 * K2_T] = rc_s[1] * p.inv_dt;
+    gq[20 * K2_T] = rc_s[2] * p.inv_dt;
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
@@ -155,7 +160,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
       const int s = link_s(a), r = link_r(a);
       const double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
       const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) * sc;  // arm length in samples
-      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : len;        // light travel time of link +a
+      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : len;        // light travel time of link +a (KEPLER1, TABLE: |r_r - r_s|/c)
       gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : len;    // of link -a
       gq[(17 + a) * K2_T] = 1.0 / len;  // n_a = (offset_r - offset_s) / len
     }
@@ -198,6 +203,11 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
         const double2 g0 = GEO2(0), g1 = GEO2(1);
         Dc[0] = fma(kx, g0.x, ky * g1.x);
         Dc[1] = fma(kx, g0.y, ky * g1.y);
+        if (KIND == 2) {  // the centroid of a tabulated orbit has a z component
+          const double2 g2 = GEO2(20);
+          Dc[0] = fma(kz, g2.x, Dc[0]);
+          Dc[1] = fma(kz, g2.y, Dc[1]);
+        }
       }
       // per spacecraft slot: k.offset, u.offset, v.offset (samples) and the reception-time
       // reads h(t - k.r_r/c).  The loops below are NOT unrolled (the unrolled body overflowed
@@ -305,6 +315,9 @@ static int launch_k2(const K2Params& p, cudaStream_t st) {
   if (p.orb.kind == 0) {
     LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k2_link_response<HT, 0><<<grid, K2_THREADS, smem, st>>>(p);
+  } else if (p.orb.kind == 2) {
+    LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k2_link_response<HT, 2><<<grid, K2_THREADS, smem, st>>>(p);
   } else {
     LISA_CUDA(cudaFuncSetAttribute(k2_link_response<HT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k2_link_response<HT, 1><<<grid, K2_THREADS, smem, st>>>(p);
@@ -326,7 +339,7 @@ int run_link_response(int B, long long N, double t0, double dt, int order, long 
   p.orb = orb;
   p.group = B < K2_G ? B : K2_G;
   // |K - Kc| <= |Dl| + drift of Dc over the tile + 1.5; the pair window adds half + 1
-  p.halo = (int)ceil((orb.max_off_over_c + orb.max_L) / dt + orb.a_over_c * orb.w * K2_T + 1.5) + p.half + 2;
+  p.halo = (int)ceil((orb.max_off_over_c + orb.max_L) / dt + orb.max_dc_rate * K2_T + 1.5) + p.half + 2;
   make_lags(order, &p.ls);
   if (!g_force_generic) {
     switch (p.half) {

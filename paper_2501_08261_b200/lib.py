@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblisa_td.so")
 
 EXPORTS = [
-    "lisa_td_last_error", "lisa_td_version", "lisa_td_modes_to_pol", "lisa_td_link_response",
+    "lisa_td_last_error", "lisa_td_version", "lisa_td_orbit_table_create", "lisa_td_orbit_table_destroy", "lisa_td_modes_to_pol", "lisa_td_link_response",
     "lisa_td_link_response_up2",
     "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_response_tdi_workspace_bytes",
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
@@ -38,7 +38,31 @@ class Orbit(C.Structure):
     """lisa_td_orbit"""
     _fields_ = [("kind", C.c_int), ("L_m", C.c_double), ("a_m", C.c_double),
                 ("year_s", C.c_double), ("phase0", C.c_double), ("t_ref", C.c_double),
-                ("r_static", (C.c_double * 3) * 3), ("L_static", C.c_double * 6)]
+                ("r_static", (C.c_double * 3) * 3), ("L_static", C.c_double * 6),
+                ("table", C.c_void_p)]
+
+
+class OrbitTable:
+    """lisa_td_orbit_table: device copy of tabulated spacecraft positions [n_tab][3][3] (metres)."""
+
+    def __init__(self, r_tab, t_tab0, dt_tab, order=7):
+        r = np.ascontiguousarray(r_tab, dtype=np.float64)
+        if r.ndim != 3 or r.shape[1:] != (3, 3):
+            raise ValueError("r_tab must be [n_tab][3][3]")
+        self._h = C.c_void_p()
+        _check(load().lisa_td_orbit_table_create(C.byref(self._h), r.shape[0], float(t_tab0), float(dt_tab),
+                                                 int(order), r.ctypes.data_as(C.c_void_p)))
+
+    def close(self):
+        if self._h:
+            load().lisa_td_orbit_table_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def make_orbit(d: dict) -> Orbit:
@@ -54,6 +78,12 @@ def make_orbit(d: dict) -> Orbit:
         o.kind = 1
         o.L_m, o.a_m, o.year_s = float(d["L_m"]), float(d["a_m"]), float(d["year_s"])
         o.phase0, o.t_ref = float(d.get("phase0", 0.0)), float(d.get("t_ref", 0.0))
+    elif d["kind"] == "table":
+        # the handle (device copy) is created once and cached in the description
+        if "_lisa_table" not in d:
+            d["_lisa_table"] = OrbitTable(d["r_tab"], d["t_tab0"], d["dt_tab"], d.get("tab_order", 7))
+        o.kind = 2
+        o.table = d["_lisa_table"]._h
     else:
         raise ValueError(d["kind"])
     return o
@@ -73,6 +103,8 @@ def load() -> C.CDLL:
     vp, dbl, i32, i64 = C.c_void_p, C.c_double, C.c_int, C.c_longlong
     L.lisa_td_last_error.restype = C.c_char_p
     L.lisa_td_version.restype = i32
+    L.lisa_td_orbit_table_create.argtypes = [C.POINTER(vp), i32, dbl, dbl, i32, vp]
+    L.lisa_td_orbit_table_destroy.argtypes = [vp]
     L.lisa_td_modes_to_pol.argtypes = [i32, i64, i32, C.POINTER(i32), C.POINTER(i32)] + [vp] * 11 + [vp]
     L.lisa_td_link_response.argtypes = [i32, i64, dbl, dbl, i32, i64, vp, vp, vp, vp,
                                         C.POINTER(Orbit), vp, vp]

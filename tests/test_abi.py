@@ -34,8 +34,8 @@ def test_version_and_error_string(lib):
 
 
 def test_orbit_struct_layout_matches_header(lib):
-    # int + pad, 5 doubles, 9 doubles, 6 doubles
-    assert C.sizeof(lib.Orbit) == 8 + 5 * 8 + 9 * 8 + 6 * 8
+    # int + pad, 5 doubles, 9 doubles, 6 doubles, one pointer
+    assert C.sizeof(lib.Orbit) == 8 + 5 * 8 + 9 * 8 + 6 * 8 + 8
 
 
 def test_argument_validation_happens_before_any_launch(lib):
