@@ -32,6 +32,8 @@ class OrcOrbit(C.Structure):
         ("t_tab0", C.c_double),
         ("dt_tab", C.c_double),
         ("r_tab", C.POINTER(C.c_double)),
+        ("tt_order", C.c_int),
+        ("nested", C.c_int),
     ]
 
 
@@ -63,6 +65,8 @@ def make_orbit(d: dict) -> OrcOrbit:
         o.r_tab = tab.ctypes.data_as(C.POINTER(C.c_double))
     else:
         raise ValueError(d["kind"])
+    o.tt_order = int(d.get("tt_order", 0))  # reading A22
+    o.nested = int(d.get("nested", 0))
     return o
 
 
@@ -88,6 +92,11 @@ class Oracle:
         L.orc_wigner_small_d.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _dp]
         L.orc_swsh.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp]
         L.orc_orbit_eval.argtypes = [C.POINTER(OrcOrbit), C.c_double, _dp, _dp]
+        L.orc_orbit_state.argtypes = [C.POINTER(OrcOrbit), C.c_double, _dp, _dp]
+        L.orc_nested_delay.restype = C.c_double
+        L.orc_nested_delay.argtypes = [C.POINTER(OrcOrbit), C.c_double, _ip, C.c_int]
+        L.orc_laser_links3.argtypes = [C.c_long, C.c_double, C.c_double, C.c_int, C.c_long, _dp,
+                                       C.POINTER(OrcOrbit), _dp]
         L.orc_modes_to_pol.argtypes = [C.c_int, C.c_long, C.c_int, _ip, _ip] + [_dp] * 9 + [
             C.c_long, C.c_long, _dp, _dp]
         L.orc_link_response.argtypes = [C.c_int, C.c_long, C.c_double, C.c_double, C.c_int,
@@ -145,6 +154,18 @@ class Oracle:
         self.lib.orc_orbit_eval(C.byref(o), float(t), _p(r), _p(L))
         return r.reshape(3, 3), L
 
+    def orbit_state(self, orbit, t):
+        o = make_orbit(orbit)
+        r = np.zeros(9)
+        v = np.zeros(9)
+        self.lib.orc_orbit_state(C.byref(o), float(t), _p(r), _p(v))
+        return r.reshape(3, 3), v.reshape(3, 3)
+
+    def nested_delay(self, orbit, t, labels):
+        o = make_orbit(orbit)
+        lab = np.ascontiguousarray(labels, dtype=np.int32)
+        return self.lib.orc_nested_delay(C.byref(o), float(t), lab.ctypes.data_as(_ip), lab.size)
+
     # -- stages -------------------------------------------------------------
     @staticmethod
     def _modes(l, m):
@@ -187,6 +208,15 @@ class Oracle:
         o = make_orbit(orbit)
         y = np.zeros((6, p.size))
         rc = self.lib.orc_laser_links(p.size, t0, dt, order, margin, _p(p), C.byref(o), _p(y))
+        assert rc == 0, rc
+        return y
+
+    def laser_links3(self, p3, orbit, t0, dt, order, margin):
+        p3 = _f64(p3)
+        assert p3.ndim == 2 and p3.shape[0] == 3
+        o = make_orbit(orbit)
+        y = np.zeros((6, p3.shape[1]))
+        rc = self.lib.orc_laser_links3(p3.shape[1], t0, dt, order, margin, _p(p3), C.byref(o), _p(y))
         assert rc == 0, rc
         return y
 

@@ -4,7 +4,7 @@
  * A plain, slow, obviously-correct evaluation of the per-likelihood hot path of
  * arXiv:2501.08261 ("GPU-accelerated LISA parameter estimation with full time
  * domain response"), written from the paper's equations and from the
- * readings A1..A18 listed in DESIGN.md / SURVEY.md section 8(c).
+ * readings A1..A22 listed in DESIGN.md / SURVEY.md section 8(c).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
  * reference legs may build, load or call this file.  It shares no code, header,
@@ -38,6 +38,11 @@
  *                            midpoint error of a quadratic
  *   F1  orc_fisher         : linear-model closed form via Parseval (time-domain Gram matrix),
  *                            symmetry, step independence, Hessian of orc_loglike
+ *   A22 tt_order / nested  : velocity = d/dt position, first-order travel time vs the fixed point of
+ *                            c L = |r_r(t) - r_s(t - L)|, chained delay vs the light path traced
+ *                            leg by leg, nested == summed on a static constellation, and
+ *                            three-laser cancellation on flexing arms (chained X2 at the 1e-13
+ *                            floor, chained X1.5 and summed X2 at 1e-8)
  * No function is "parity unpinned".
  */
 #include <math.h>
@@ -85,6 +90,15 @@ typedef struct {
   int n_tab, tab_order;  /* tab_order odd: tab_order + 1 interpolation nodes */
   double t_tab0, dt_tab;
   const double* r_tab;   /* [n_tab][3][3] metres */
+  /* Delay model (reading A22 of DESIGN.md).
+   * tt_order 0: L_l(t) = |r_r(t) - r_s(t)| / c (reading A8).
+   * tt_order 1: first order in v/c of  c L = |r_r(t) - r_s(t - L)|:
+   *             L_l(t) = (d/c) (1 + n.v_s/c),  d = |r_r - r_s|, n = (r_r - r_s)/d, v_s = sender
+   *             velocity, all at the reception time t (so L_l != L_{-l}).  STATIC ignores it.
+   * nested 0: TDI delays are sums of L_l(t), all at the output time (reading A10).
+   * nested 1: TDI delays are chained along the light path traced back from the output time:
+   *           tau_0 = 0, tau_{i+1} = tau_i + L_{l_i}(t - tau_i). */
+  int tt_order, nested;
 } orc_orbit;
 
 /* Link order l = [1,2,3,-1,-2,-3]; (sender, receiver) spacecraft, 1-based
@@ -269,20 +283,24 @@ int orc_modes_to_pol(int B, long N, int n_modes, const int* l, const int* m, con
 
 /* --------------------------------------------------------------- orbits -- */
 
-/* Positions r[3][3] (metres) and light travel times L[6] (seconds, link order) at time t.
- * STATIC: as given.  KEPLER1: reading A8 (first-order solution of Kepler's equation). */
-static void orbit_eval(const orc_orbit* o, REAL t, REAL r[3][3], REAL L[6]) {
+/* Positions r[3][3] (metres) and velocities v[3][3] (m/s) at time t.
+ * STATIC: as given, at rest.  KEPLER1: reading A8 (first-order solution of Kepler's equation)
+ * and its time derivative.  TABLE: reading A21 and the derivative of the interpolant. */
+static void orbit_state(const orc_orbit* o, REAL t, REAL r[3][3], REAL v[3][3]) {
   if (o->kind == 0) {
     for (int i = 0; i < 3; ++i)
-      for (int j = 0; j < 3; ++j) r[i][j] = (REAL)o->r_static[i][j];
-    for (int k = 0; k < 6; ++k) L[k] = (REAL)o->L_static[k];
+      for (int j = 0; j < 3; ++j) {
+        r[i][j] = (REAL)o->r_static[i][j];
+        v[i][j] = 0;
+      }
     return;
   }
   if (o->kind == 2) {
     /* TABLE (orbits "tracked over the whole observation period", ESA-style file;
      * reading A21): Lagrange interpolation of degree q = tab_order on the q+1 nodes
-     * j0 .. j0+q,  j0 = floor(u) - (q-1)/2 clamped to [0, n_tab-q-1],  u = (t - t_tab0)/dt_tab;
-     * light travel times L_l = |r_r - r_s| / c as for KEPLER1. */
+     * j0 .. j0+q,  j0 = floor(u) - (q-1)/2 clamped to [0, n_tab-q-1],  u = (t - t_tab0)/dt_tab.
+     * Velocity = d/dt of the same polynomial:  c_i'(x) = sum_{k != i} [prod_{m != i,k} (x - m)] /
+     * prod_{m != i} (i - m), divided by dt_tab. */
     int q = o->tab_order;
     REAL u = (t - (REAL)o->t_tab0) / (REAL)o->dt_tab;
     long j0 = (long)floor(u) - (q - 1) / 2;
@@ -290,19 +308,28 @@ static void orbit_eval(const orc_orbit* o, REAL t, REAL r[3][3], REAL L[6]) {
     if (j0 > o->n_tab - q - 1) j0 = o->n_tab - q - 1;
     REAL x = u - (REAL)j0;
     for (int k = 0; k < 3; ++k)
-      for (int j = 0; j < 3; ++j) r[k][j] = 0;
+      for (int j = 0; j < 3; ++j) r[k][j] = v[k][j] = 0;
     for (int i = 0; i <= q; ++i) {
-      REAL c = 1;
+      REAL c = 1, den = 1, dc = 0;
       for (int m = 0; m <= q; ++m)
-        if (m != i) c *= (x - (REAL)m) / (REAL)(i - m);
+        if (m != i) {
+          c *= (x - (REAL)m) / (REAL)(i - m);
+          den *= (REAL)(i - m);
+        }
+      for (int k = 0; k <= q; ++k) {
+        if (k == i) continue;
+        REAL pr = 1;
+        for (int m = 0; m <= q; ++m)
+          if (m != i && m != k) pr *= x - (REAL)m;
+        dc += pr;
+      }
+      dc /= den * (REAL)o->dt_tab;
       for (int k = 0; k < 3; ++k)
-        for (int j = 0; j < 3; ++j) r[k][j] += c * (REAL)o->r_tab[((size_t)(j0 + i) * 3 + k) * 3 + j];
-    }
-    for (int k = 0; k < 6; ++k) {
-      const REAL* rs = r[LINK_S[k] - 1];
-      const REAL* rr = r[LINK_R[k] - 1];
-      REAL d0 = rr[0] - rs[0], d1 = rr[1] - rs[1], d2 = rr[2] - rs[2];
-      L[k] = sqrt(d0 * d0 + d1 * d1 + d2 * d2) / ORC_C_LIGHT;
+        for (int j = 0; j < 3; ++j) {
+          REAL rij = (REAL)o->r_tab[((size_t)(j0 + i) * 3 + k) * 3 + j];
+          r[k][j] += c * rij;
+          v[k][j] += dc * rij;
+        }
     }
     return;
   }
@@ -312,24 +339,75 @@ static void orbit_eval(const orc_orbit* o, REAL t, REAL r[3][3], REAL L[6]) {
   REAL e = sqrt(1 + 2 * delta / sq3 + 4 * delta * delta / 3) - 1;
   REAL inc = atan(delta / (1 + delta / sq3));
   REAL ci = cos(inc), si = sin(inc);
+  REAL w = 2 * ORC_PI / (REAL)o->year_s; /* dM/dt */
   for (int k = 0; k < 3; ++k) {
     REAL sigma = 2 * ORC_PI * (REAL)k / 3;
     REAL M = 2 * ORC_PI * (t - (REAL)o->t_ref) / (REAL)o->year_s - sigma - (REAL)o->phase0;
     REAL psi = M + e * sin(M);
+    REAL dpsi = w * (1 + e * cos(M)); /* d psi / dt */
     REAL x = a * (cos(psi) - e) * ci;
     REAL y = a * sqrt(1 - e * e) * sin(psi);
     REAL z = a * (cos(psi) - e) * si;
+    REAL vx = -a * sin(psi) * dpsi * ci;
+    REAL vy = a * sqrt(1 - e * e) * cos(psi) * dpsi;
+    REAL vz = -a * sin(psi) * dpsi * si;
     REAL cs = cos(sigma), ss = sin(sigma);
     r[k][0] = cs * x - ss * y;
     r[k][1] = ss * x + cs * y;
     r[k][2] = z;
+    v[k][0] = cs * vx - ss * vy;
+    v[k][1] = ss * vx + cs * vy;
+    v[k][2] = vz;
+  }
+}
+
+/* Positions r[3][3] (metres) and light travel times L[6] (seconds, link order) at time t.
+ * STATIC: as given.  Otherwise L_l = d/c (tt_order 0, reading A8) or (d/c)(1 + n.v_s/c)
+ * (tt_order 1, reading A22), d = |r_r - r_s|, n from sender to receiver. */
+static void orbit_eval(const orc_orbit* o, REAL t, REAL r[3][3], REAL L[6]) {
+  REAL v[3][3];
+  orbit_state(o, t, r, v);
+  if (o->kind == 0) {
+    for (int k = 0; k < 6; ++k) L[k] = (REAL)o->L_static[k];
+    return;
   }
   for (int k = 0; k < 6; ++k) {
     const REAL* rs = r[LINK_S[k] - 1];
     const REAL* rr = r[LINK_R[k] - 1];
+    const REAL* vs = v[LINK_S[k] - 1];
     REAL d0 = rr[0] - rs[0], d1 = rr[1] - rs[1], d2 = rr[2] - rs[2];
-    L[k] = sqrt(d0 * d0 + d1 * d1 + d2 * d2) / ORC_C_LIGHT;
+    REAL d = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+    L[k] = d / ORC_C_LIGHT;
+    if (o->tt_order == 1) {
+      REAL nv = (d0 * vs[0] + d1 * vs[1] + d2 * vs[2]) / d;
+      L[k] = (d / ORC_C_LIGHT) * (1 + nv / ORC_C_LIGHT);
+    }
   }
+}
+
+void orc_orbit_state(const orc_orbit* o, double t, double* r9, double* v9) {
+  REAL r[3][3], v[3][3];
+  orbit_state(o, (REAL)t, r, v);
+  for (int i = 0; i < 9; ++i) {
+    r9[i] = (double)r[i / 3][i % 3];
+    v9[i] = (double)v[i / 3][i % 3];
+  }
+}
+
+/* Chained delay (seconds) of the signed link labels lab[0..n) applied in this order, starting
+ * at time t (reading A22):  tau_0 = 0,  tau_{i+1} = tau_i + L_{lab_i}(t - tau_i). */
+static int link_index(int link);
+static REAL nested_delay(const orc_orbit* o, REAL t, const int* lab, int n) {
+  REAL tau = 0;
+  for (int i = 0; i < n; ++i) {
+    REAL r[3][3], L[6];
+    orbit_eval(o, t - tau, r, L);
+    tau += L[link_index(lab[i])];
+  }
+  return tau;
+}
+double orc_nested_delay(const orc_orbit* o, double t, const int* lab, int n) {
+  return (double)nested_delay(o, (REAL)t, lab, n);
 }
 
 void orc_orbit_eval(const orc_orbit* o, double t, double* r9, double* L6) {
@@ -499,6 +577,29 @@ int orc_laser_links(long N, double t0, double dt, int order, long margin, const 
   return 0;
 }
 
+/* Three independent lasers, one per spacecraft (used to pin the chaining order of A22):
+ * y_{slr}[n] = p_s(n - L_l(t_n)/dt) - p_r[n]; p: [3][N]; zero outside [margin, N-margin). */
+int orc_laser_links3(long N, double t0, double dt, int order, long margin, const double* p,
+                     const orc_orbit* orbit, double* y) {
+  REAL* pr = (REAL*)malloc((size_t)3 * N * sizeof(REAL));
+  if (!pr) return -3;
+  for (long i = 0; i < 3 * N; ++i) pr[i] = (REAL)p[i];
+#pragma omp parallel for schedule(static)
+  for (long n = 0; n < N; ++n) {
+    if (n < margin || n >= N - margin) {
+      for (int l = 0; l < 6; ++l) y[(size_t)l * N + n] = 0;
+      continue;
+    }
+    REAL r[3][3], L[6];
+    orbit_eval(orbit, (REAL)t0 + (REAL)n * (REAL)dt, r, L);
+    for (int l = 0; l < 6; ++l)
+      y[(size_t)l * N + n] = (double)(delay_read(pr + (size_t)(LINK_S[l] - 1) * N, N, n, L[l] / (REAL)dt, order) -
+                                      pr[(size_t)(LINK_R[l] - 1) * N + n]);
+  }
+  free(pr);
+  return 0;
+}
+
 /* ------------------------------------------------------------------ S3 -- */
 
 /* Term tables for the Michelson X.  Links are signed labels
@@ -534,6 +635,38 @@ static const tdi_term X20_TERMS[16] = {
     {-1, -2, {3, -3, -2, 2, 0}},
 };
 
+/* The same terms with the delay labels in CHAINING order (reading A22): the label nearest to the
+ * output time first.  X compares the two light paths that leave spacecraft 1, visit 2 and 3 in
+ * opposite orders (twice each for generation 2) and return to 1.  Traced BACK from the output time
+ * t at spacecraft 1, link by link (link l is received at LINK_R[l], so stepping back along it
+ * lands on LINK_S[l]), the two paths are
+ *     path A: 3, -3, -2, 2, -2, 2, 3, -3      (1 <- 2 <- 1 <- 3 <- 1 <- 3 <- 1 <- 2 <- 1)
+ *     path B: -2, 2, 3, -3, 3, -3, -2, 2      (1 <- 3 <- 1 <- 2 <- 1 <- 2 <- 1 <- 3 <- 1)
+ * and every delay of Eq. 2.9 / 2.10 is, as a multiset, a leading piece of one of them, applied to
+ * the link measured at the spacecraft that piece ends on.  Written out term by term: */
+static const tdi_term X15_NESTED[8] = {
+    {+1, -3, {-2, 2, 3, 0}}, {-1, -3, {3, 0}},          {+1, 3, {-2, 2, 0}}, {-1, 3, {0}},
+    {+1, 2, {-2, 0}},        {-1, 2, {3, -3, -2, 0}},   {+1, -2, {0}},       {-1, -2, {3, -3, 0}},
+};
+static const tdi_term X20_NESTED[16] = {
+    {+1, -3, {-2, 2, 3, 0}},
+    {-1, -3, {3, 0}},
+    {+1, -3, {-2, 2, 3, -3, 3, 0}},
+    {-1, -3, {3, -3, -2, 2, -2, 2, 3, 0}},
+    {+1, 3, {-2, 2, 0}},
+    {-1, 3, {0}},
+    {+1, 3, {-2, 2, 3, -3, 0}},
+    {-1, 3, {3, -3, -2, 2, -2, 2, 0}},
+    {+1, 2, {-2, 0}},
+    {-1, 2, {3, -3, -2, 0}},
+    {+1, 2, {-2, 2, 3, -3, 3, -3, -2, 0}},
+    {-1, 2, {3, -3, -2, 2, -2, 0}},
+    {+1, -2, {0}},
+    {-1, -2, {3, -3, 0}},
+    {+1, -2, {-2, 2, 3, -3, 3, -3, 0}},
+    {-1, -2, {3, -3, -2, 2, 0}},
+};
+
 /* cyclic relabelling 1->2->3->1 of |link|, sign kept */
 static int cyc(int link, int times) {
   int s = link < 0 ? -1 : 1, a = link < 0 ? -link : link;
@@ -543,12 +676,14 @@ static int cyc(int link, int times) {
 static int link_index(int link) { return link > 0 ? link - 1 : -link + 2; }
 
 /* y: [B][6][N] REAL -> tdi: [B][3][N] REAL, XYZ (out_kind 0) or AET (1).
- * generation 15 or 20.  All L at the output time t, delays summed not nested (A10).
+ * generation 15 or 20.  All L at the output time t, delays summed not nested (A10), unless
+ * orbit->nested (A22).
  * Outputs are zero outside [margin_lo, N - margin_hi). */
 static void s3_core(int B, long N, REAL t0, REAL dt, int order, int generation, int out_kind,
                     long margin_lo, long margin_hi, const REAL* y, const orc_orbit* orbit,
                     long n_lo, long n_hi, REAL* tdi) {
   const tdi_term* terms = generation == 15 ? X15_TERMS : X20_TERMS;
+  if (orbit->nested) terms = generation == 15 ? X15_NESTED : X20_NESTED;
   int n_terms = generation == 15 ? 8 : 16;
   for (int b = 0; b < B; ++b) {
     const REAL* yb = y + (size_t)b * 6 * N;
@@ -566,8 +701,14 @@ static void s3_core(int B, long N, REAL t0, REAL dt, int order, int generation, 
         REAL acc = 0;
         for (int k = 0; k < n_terms; ++k) {
           REAL D = 0;
-          for (int q = 0; terms[k].delays[q] != 0; ++q)
-            D += L[link_index(cyc(terms[k].delays[q], c))];
+          if (orbit->nested) { /* A22: chained along the light path */
+            int lab[8], nl = 0;
+            for (int q = 0; terms[k].delays[q] != 0; ++q) lab[nl++] = cyc(terms[k].delays[q], c);
+            D = nested_delay(orbit, t0 + (REAL)n * dt, lab, nl);
+          } else { /* A10: summed, every L at the output time */
+            for (int q = 0; terms[k].delays[q] != 0; ++q)
+              D += L[link_index(cyc(terms[k].delays[q], c))];
+          }
           D /= dt;
           const REAL* series = yb + (size_t)link_index(cyc(terms[k].link, c)) * N;
           acc += (REAL)terms[k].sign * delay_read(series, N, n, D, order);
