@@ -338,6 +338,31 @@ def run_ours(args):
                 "ms_s1_plus_s2_full_rate": stage_ms["S1_modes_to_pol"] + stage_ms["S2_link_response"],
                 "cite": "PAPER.md:243 (10 s sampling, linear interpolation), DESIGN.md reading A20"}
     del c_in, hpc, hcc
+    # ---- first-order light travel times + TDI delays chained along the light path
+    # (reading A22): S2 and S3 with that delay model (restores y, tdi of the default model after)
+    orb22 = dict(inp["orbit"], tt_order=1, nested=1)
+
+    def nested_s2():
+        lib.link_response(B, N, t0, dt, ORDER, inp["margin_y"], hp, hc, g("lam"), g("beta_sky"), orb22, y)
+
+    def nested_s3():
+        lib.tdi2(B, N, t0, dt, ORDER, 20, 1, inp["margin_lo"], inp["margin_hi"], y, orb22, tdi)
+    for _ in range(3):
+        nested_s2(); nested_s3()
+    ne = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ne[0].record()
+    for _ in range(5):
+        nested_s2()
+    ne[1].record()
+    for _ in range(5):
+        nested_s3()
+    ne[2].record()
+    torch.cuda.synchronize()
+    nested_info = {"ms_s2_tt_order1": ne[0].elapsed_time(ne[1]) / 5, "ms_s3_chained": ne[1].elapsed_time(ne[2]) / 5,
+                   "ms_s2_default": stage_ms["S2_link_response"], "ms_s3_default": stage_ms["S3_tdi2"],
+                   "cite": "PAPER.md:163, 380-384; DESIGN.md reading A22"}
+    s2(); s3()
+    torch.cuda.synchronize()
     fisher_info = {"D": D, "walkers": D + 1, "ms_per_matrix": fe[0].elapsed_time(fe[1]) / 5,
                    "ms_fft_plus_k6": fe[1].elapsed_time(fe[2]) / 5,
                    "cite": "PAPER.md:249 (first-order finite differences), DESIGN.md reading A19"}
@@ -410,7 +435,7 @@ def run_ours(args):
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
-        "next": {"fisher": fisher_info, "up2": up2_info},
+        "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info},
     }
     print(json.dumps(line))
     plan.close()

@@ -9,7 +9,7 @@
  *   S5  inner products -> log L      Eq. 2.12-2.13 (band PAPER.md:243)
  *
  * The readings taken where the paper is silent or garbled are listed in DESIGN.md section 2
- * (A1..A18); the comments below name the ones each call depends on.
+ * (A1..A22); the comments below name the ones each call depends on.
  *
  * General conventions
  *  - Every array pointer is a DEVICE pointer unless its name ends in _host.  All arrays are
@@ -66,7 +66,20 @@ LISA_TD_API int lisa_td_version(void);
  *                   grid, held in a lisa_td_orbit_table; per sample they are interpolated with a
  *                   Lagrange polynomial of odd degree q on the q+1 nodes j0..j0+q,
  *                   j0 = floor((t - t_tab0)/dt_tab) - (q-1)/2 clamped to the table;
- *                   L_l(t) = |r_r(t) - r_s(t)|/c.  The table must cover [t0, t0 + N dt]. */
+ *                   L_l(t) = |r_r(t) - r_s(t)|/c.  The table must cover [t0, t0 + N dt].
+ *
+ * Delay model (reading A22 of DESIGN.md):
+ * tt_order   0: L_l(t) = |r_r(t) - r_s(t)|/c as above.
+ *            1: first order in v/c of  c L = |r_r(t) - r_s(t - L)|:
+ *               L_l(t) = (d/c)(1 + n.v_s/c), d = |r_r - r_s|, n = (r_r - r_s)/d, v_s = velocity of the
+ *               sender (analytic for KEPLER1, derivative of the interpolant for TABLE), all at the
+ *               reception time t, so that L_l != L_{-l}.  Used by S2, S3 and the laser helper.
+ *               STATIC ignores it (its six L are given).
+ * tdi_nested 0: every TDI delay is the SUM of the listed L_l(t_n), all at the output time (A10).
+ *            1: every TDI delay is CHAINED along the light path traced back from the output time:
+ *               tau_0 = 0, tau_{i+1} = tau_i + L_{l_i}(t_n - tau_i), labels in the order of the two
+ *               paths 1<-2<-1<-3<-1<-3<-1<-2<-1 and 1<-3<-1<-2<-1<-2<-1<-3<-1 (for X; Y, Z cyclic),
+ *               of which every delay of Eq. 2.9 / 2.10 is a leading piece.  S3 only. */
 typedef struct lisa_td_orbit_table lisa_td_orbit_table;
 typedef struct {
   int kind;
@@ -74,6 +87,8 @@ typedef struct {
   double r_static[3][3];
   double L_static[6];
   const lisa_td_orbit_table* table; /* kind 2 only */
+  int tt_order;                     /* 0 | 1 */
+  int tdi_nested;                   /* 0 | 1 */
 } lisa_td_orbit;
 
 /* Owns a device copy of the table (the only device memory the library holds besides plans).

@@ -104,8 +104,21 @@ struct lisa_td_orbit_table {
 
 namespace lisa {
 
+static int make_orbit_dev_kind(const lisa_td_orbit* o, OrbitDev* d);
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* d) {
   if (!o) return set_error(LISA_TD_EINVAL, "orbit_host is NULL");
+  if ((o->tt_order != 0 && o->tt_order != 1) || (o->tdi_nested != 0 && o->tdi_nested != 1))
+    return set_error(LISA_TD_EINVAL, "orbit: tt_order=%d and tdi_nested=%d must be 0 or 1", o->tt_order, o->tdi_nested);
+  int rc = make_orbit_dev_kind(o, d);
+  if (rc) return rc;
+  d->nested = o->tdi_nested;
+  if (o->kind != 0 && o->tt_order) {  // A22: L = (d/c)(1 + n.v/c), |v|/c < 1.2e-4 for any heliocentric 1 AU orbit
+    d->tt_order = 1;
+    d->max_L *= 1.0 + 1.2e-4;
+  }
+  return LISA_TD_OK;
+}
+static int make_orbit_dev_kind(const lisa_td_orbit* o, OrbitDev* d) {
   memset(d, 0, sizeof(*d));
   d->kind = o->kind;
   if (o->kind == 2) {

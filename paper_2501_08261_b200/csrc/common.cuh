@@ -74,6 +74,8 @@ struct OrbitDev {
   int n_tab, tab_order;
   double t_tab0, inv_dt_tab;
   double tab_w[16];               // 1 / prod_{m != i} (i - m), i = 0..tab_order
+  // delay model (reading A22): first-order light travel times, TDI delays chained along the path
+  int tt_order, nested;
 };
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* out);
 
@@ -126,7 +128,10 @@ __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
 // ------------------------------------------------------------------ orbit evaluation
 // TABLE: Lagrange interpolation of degree q on the nodes j0..j0+q, j0 = floor(u) - (q-1)/2
 // clamped to the table, u = (t - t_tab0)/dt_tab (reading A21); the common part is the centroid.
-__device__ __forceinline__ void orbit_table_eval(const OrbitDev& o, double t, double (&d)[3][3], double (&rc_s)[3]) {
+// WITH_V: also the velocities v[k][xyz] [m/s], the derivative of the same interpolant.
+template <bool WITH_V>
+__device__ __forceinline__ void orbit_table_eval(const OrbitDev& o, double t, double (&d)[3][3], double (&rc_s)[3],
+                                                 double (&v)[3][3]) {
   const int q = o.tab_order;
   const double u = (t - o.t_tab0) * o.inv_dt_tab;
   int j0 = (int)floor(u) - (q - 1) / 2;
@@ -136,18 +141,30 @@ __device__ __forceinline__ void orbit_table_eval(const OrbitDev& o, double t, do
 #pragma unroll
   for (int k = 0; k < 3; ++k)
 #pragma unroll
-    for (int j = 0; j < 3; ++j) r[k][j] = 0.0;
+    for (int j = 0; j < 3; ++j) {
+      r[k][j] = 0.0;
+      if (WITH_V) v[k][j] = 0.0;
+    }
 #pragma unroll 1
   for (int i = 0; i <= q; ++i) {
-    double c = o.tab_w[i];
+    double c = o.tab_w[i], dc = 0.0;  // c = w_i prod (x - m), dc = its x-derivative (product rule, running)
 #pragma unroll 1
     for (int m = 0; m <= q; ++m)
-      if (m != i) c *= x - (double)m;
+      if (m != i) {
+        const double g = x - (double)m;
+        if (WITH_V) dc = fma(dc, g, c);
+        c *= g;
+      }
     const double* row = o.tab + (size_t)(j0 + i) * 9;
+    if (WITH_V) dc *= o.inv_dt_tab;
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) r[k][j] = fma(c, __ldg(row + 3 * k + j), r[k][j]);
+      for (int j = 0; j < 3; ++j) {
+        const double rij = __ldg(row + 3 * k + j);
+        r[k][j] = fma(c, rij, r[k][j]);
+        if (WITH_V) v[k][j] = fma(dc, rij, v[k][j]);
+      }
   }
 #pragma unroll
   for (int j = 0; j < 3; ++j) {
@@ -161,18 +178,23 @@ __device__ __forceinline__ void orbit_table_eval(const OrbitDev& o, double t, do
 // d[k][xyz]: spacecraft positions minus a common part; rc_s: that common part as a light
 // travel time [s] per unit direction.  KEPLER1: common part a(cos M, sin M, 0); STATIC: zero
 // (d = the positions themselves); TABLE: the centroid.
-__device__ __forceinline__ void orbit_offsets(const OrbitDev& o, double t, double (&d)[3][3],
-                                              double (&rc_s)[3]) {
+// WITH_V: also the (full, not split) velocities v[k][xyz] [m/s] (reading A22).
+template <bool WITH_V>
+__device__ __forceinline__ void orbit_offsets_v(const OrbitDev& o, double t, double (&d)[3][3],
+                                                double (&rc_s)[3], double (&v)[3][3]) {
   if (o.kind == 0) {
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) d[k][j] = o.r[k][j];
+      for (int j = 0; j < 3; ++j) {
+        d[k][j] = o.r[k][j];
+        if (WITH_V) v[k][j] = 0.0;
+      }
     rc_s[0] = rc_s[1] = rc_s[2] = 0.0;
     return;
   }
   if (o.kind == 2) {
-    orbit_table_eval(o, t, d, rc_s);
+    orbit_table_eval<WITH_V>(o, t, d, rc_s, v);
     return;
   }
   double cM, sM;
@@ -198,7 +220,21 @@ __device__ __forceinline__ void orbit_offsets(const OrbitDev& o, double t, doubl
     d[k][0] = o.a * fma(o.cs[k], px, -o.sn[k] * py);
     d[k][1] = o.a * fma(o.sn[k], px, o.cs[k] * py);
     d[k][2] = o.a * o.si * (cMk + u1);
+    if (WITH_V) {
+      // d psi_k/dt = w (1 + e cos M_k);  (x, y, z)' = a (-sin psi ci, bq cos psi, -sin psi si) psi'
+      const double aw = o.a * o.w * fma(o.e, cMk, 1.0);
+      const double sp = sMk + ds, cp = cMk + dc;
+      const double vx = -aw * sp * o.ci, vy = aw * o.bq * cp;
+      v[k][0] = fma(o.cs[k], vx, -o.sn[k] * vy);
+      v[k][1] = fma(o.sn[k], vx, o.cs[k] * vy);
+      v[k][2] = -aw * sp * o.si;
+    }
   }
+}
+__device__ __forceinline__ void orbit_offsets(const OrbitDev& o, double t, double (&d)[3][3],
+                                              double (&rc_s)[3]) {
+  double v[3][3];
+  orbit_offsets_v<false>(o, t, d, rc_s, v);
 }
 
 // Light travel times of the six links at time t (link order [1,2,3,-1,-2,-3]).
@@ -208,15 +244,22 @@ __device__ __forceinline__ void orbit_arm_times(const OrbitDev& o, double t, dou
     for (int l = 0; l < 6; ++l) L[l] = o.L[l];
     return;
   }
-  double d[3][3], rc_s[3];
-  orbit_offsets(o, t, d, rc_s);
+  double d[3][3], rc_s[3], v[3][3];
+  if (o.tt_order) orbit_offsets_v<true>(o, t, d, rc_s, v);
+  else orbit_offsets_v<false>(o, t, d, rc_s, v);
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
     const int s = (l + 2) % 3, r = (l + 1) % 3;  // link l+1: sender, receiver
     double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
-    double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) / C_LIGHT;
+    double dist = sqrt(fma(dx, dx, fma(dy, dy, dz * dz)));
+    double len = dist / C_LIGHT;
     L[l] = len;
     L[l + 3] = len;
+    if (o.tt_order) {  // A22: (d/c)(1 + n.v_sender/c); link -(l+1) runs the other way
+      const double sc = 1.0 / (dist * C_LIGHT);
+      L[l] = fma(len, fma(dx, v[s][0], fma(dy, v[s][1], dz * v[s][2])) * sc, len);
+      L[l + 3] = fma(len, -fma(dx, v[r][0], fma(dy, v[r][1], dz * v[r][2])) * sc, len);
+    }
   }
 }
 

@@ -145,8 +145,9 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 #pragma unroll 1
   for (int c = 0; c < 2; ++c) {
     double* gq = geo + 2 * threadIdx.x + c;
-    double d[3][3], rc_s[3];
-    orbit_offsets(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s);
+    double d[3][3], rc_s[3], vel[3][3];
+    if (p.orb.tt_order) orbit_offsets_v<true>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
+    else orbit_offsets_v<false>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
     const double sc = p.inv_dt / C_LIGHT;
     gq[0 * K2_T] = rc_s[0] * p.inv_dt;   // common (1 AU) delay per unit k (samples)
     gq[1 * K2_T] = rc_s[1] * p.inv_dt;
@@ -160,8 +161,14 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
       const int s = link_s(a), r = link_r(a);
       const double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
       const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) * sc;  // arm length in samples
-      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : len;        // light travel time of link +a (KEPLER1, TABLE: |r_r - r_s|/c)
-      gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : len;    // of link -a
+      double Lp = len, Lm = len;  // light travel times of links +a, -a (KEPLER1, TABLE: |r_r - r_s|/c)
+      if (KIND != 0 && p.orb.tt_order) {  // A22: (d/c)(1 + n.v_sender/c); link -a runs r -> s
+        const double q = sc / (len * C_LIGHT);  // n.v/c = (d.v) q with d in metres, len in samples
+        Lp = fma(len, fma(dx, vel[s][0], fma(dy, vel[s][1], dz * vel[s][2])) * q, len);
+        Lm = fma(len, -fma(dx, vel[r][0], fma(dy, vel[r][1], dz * vel[r][2])) * q, len);
+      }
+      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : Lp;
+      gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : Lm;
       gq[(17 + a) * K2_T] = 1.0 / len;  // n_a = (offset_r - offset_s) / len
     }
   }

@@ -20,8 +20,8 @@ namespace lisa {
 
 struct K3Term {
   signed char sign;
-  signed char mult[6];  // multiplicity of each L_l in the delay
-  signed char pad;
+  signed char mult[6];  // multiplicity of each L_l in the delay (summed delays, A10)
+  signed char chain;    // chained delays (A22): bits 0-2 = number of legs, bit 3 = light path (0 A, 1 B)
 };
 struct K3Pair {
   int series;   // link index 0..5 of the y series
@@ -40,6 +40,7 @@ struct K3Params {
   LagW lw;
   LagS ls;
   K3Pair pair[12];  // [channel X,Y,Z][slot]
+  signed char path[3][2][8];  // chained delays: link indices of the two light paths per channel
 };
 
 // ---- term tables, restated from the paper ----------------------------------------------
@@ -71,6 +72,16 @@ static const TermSpec kX20extra[8] = {
     {-2, +1, 6, {-2, 2, 3, 3, -3, -3}},     {-2, -1, 4, {3, -3, -2, 2}},
 };
 
+// Chained delays (reading A22).  X compares two light paths that start and end on spacecraft 1.
+// Traced BACK from the output time (link l is received at link_r(l); stepping back along it lands
+// on link_s(l)) they are, as signed link labels,
+//   A: 1 <- 2 <- 1 <- 3 <- 1 <- 3 <- 1 <- 2 <- 1     B: 1 <- 3 <- 1 <- 2 <- 1 <- 2 <- 1 <- 3 <- 1
+// and every delay multiset of Eq. 2.9 / 2.10 is a leading piece of one of them, followed on that
+// path by the term's own link (checked when the tables are built): the chained delay of that term is  tau_0 = 0,
+// tau_{i+1} = tau_i + L_{path[i]}(t - tau_i)  over that piece.
+static const int kPathA[8] = {3, -3, -2, 2, -2, 2, 3, -3};
+static const int kPathB[8] = {-2, 2, 3, -3, 3, -3, -2, 2};
+
 static int cyc_label(int label, int times) {  // 1->2->3->1 on |label|, sign kept
   int s = label < 0 ? -1 : 1, a = label < 0 ? -label : label;
   for (int i = 0; i < times; ++i) a = a % 3 + 1;
@@ -78,7 +89,31 @@ static int cyc_label(int label, int times) {  // 1->2->3->1 on |label|, sign kep
 }
 static int label_index(int label) { return label > 0 ? label - 1 : -label + 2; }
 
-static void build_pairs(int generation, K3Pair* out) {
+// which path has ts.d as the multiset of its first ts.n labels: 0 (A) or 1 (B); -1 if none / both
+static int match_path(const TermSpec& ts) {
+  int hit = -1;
+  for (int c = 0; c < 2; ++c) {
+    const int* path = c == 0 ? kPathA : kPathB;
+    int cnt[6] = {0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < ts.n; ++i) {
+      cnt[label_index(path[i])]++;
+      cnt[label_index(ts.d[i])]--;
+    }
+    bool same = true;
+    for (int i = 0; i < 6; ++i) same = same && cnt[i] == 0;
+    // the term's link is the NEXT leg of the path (the beam that arrives where the piece ends);
+    // this also separates the two pieces of four legs, which are equal as multisets
+    if (same && path[ts.n] == ts.link) hit = hit == -1 ? c : -2;
+  }
+  return hit < 0 ? -1 : hit;
+}
+
+static int build_pairs(int generation, K3Pair* out, signed char (*path)[2][8]) {
+  for (int c = 0; c < 3; ++c)
+    for (int i = 0; i < 8; ++i) {
+      path[c][0][i] = (signed char)label_index(cyc_label(kPathA[i], c));
+      path[c][1][i] = (signed char)label_index(cyc_label(kPathB[i], c));
+    }
   for (int c = 0; c < 3; ++c)
     for (int slot = 0; slot < 4; ++slot) {
       K3Pair& pr = out[c * 4 + slot];
@@ -89,16 +124,19 @@ static void build_pairs(int generation, K3Pair* out) {
           const TermSpec& ts = pass == 0 ? kX15[2 * slot + k] : kX20extra[2 * slot + k];
           K3Term& t = pr.t[pr.n_terms++];
           t.sign = (signed char)ts.sign;
-          t.pad = 0;
+          const int which = match_path(ts);
+          if (which < 0) return -1;
+          t.chain = (signed char)(ts.n | (which << 3));
           for (int i = 0; i < 6; ++i) t.mult[i] = 0;
           for (int i = 0; i < ts.n; ++i) t.mult[label_index(cyc_label(ts.d[i], c))]++;
         }
       for (int k = pr.n_terms; k < 4; ++k) {
         pr.t[k].sign = 0;
-        pr.t[k].pad = 0;
+        pr.t[k].chain = 0;
         for (int i = 0; i < 6; ++i) pr.t[k].mult[i] = 0;
       }
     }
+  return 0;
 }
 
 __device__ __forceinline__ double term_delay(const K3Term& t, const double (&L)[6], double inv_dt) {
@@ -106,6 +144,44 @@ __device__ __forceinline__ double term_delay(const K3Term& t, const double (&L)[
 #pragma unroll
   for (int i = 0; i < 6; ++i) D = fma((double)t.mult[i], L[i], D);
   return D * inv_dt;
+}
+
+// Chained delays of one light path (A22): tau[i] = delay after i legs, i = 0..7, in seconds.
+__device__ __forceinline__ void chain_delays(const OrbitDev& orb, double t, const signed char (&path)[8],
+                                             double (&tau)[8]) {
+  double acc = 0.0;
+  tau[0] = 0.0;
+#pragma unroll 1
+  for (int i = 0; i < 7; ++i) {
+    double L[6];
+    orbit_arm_times(orb, t - acc, L);
+    const int l = path[i];
+    double Ll = L[0];
+#pragma unroll
+    for (int q = 1; q < 6; ++q) Ll = l == q ? L[q] : Ll;
+    acc += Ll;
+    tau[i + 1] = acc;
+  }
+}
+
+// The same chain for an ANALYTIC orbit (KEPLER1), from the six L sampled at t, t - h, t - 2h with
+// 2h = 7 max L (the longest chain): L_l(t - tau) is read off the quadratic through the three
+// samples.  Its truncation error is |d3L/dt3| x 0.064 h^3 < 1e-16 s on a heliocentric orbit (the
+// arm lengths breathe by ~1 % at the orbital rate 2e-7 rad/s), far below one ulp of the delay
+// (12 samples x 2^-52 x dt = 1.3e-14 s): 3 orbit evaluations per sample instead of 42.
+// Lq: [3][6] seconds.
+__device__ __forceinline__ void chain_delays_quad(const double* __restrict__ Lq, double inv_h,
+                                                  const signed char (&path)[8], double (&tau)[8]) {
+  double acc = 0.0;
+  tau[0] = 0.0;
+#pragma unroll
+  for (int i = 0; i < 7; ++i) {
+    const int l = path[i];
+    const double a = Lq[l], b = Lq[6 + l], c = Lq[12 + l];
+    const double x = acc * inv_h;
+    acc += fma(x * (x - 1.0), 0.5 * ((c - b) - (b - a)), fma(x, b - a, a));
+    tau[i + 1] = acc;
+  }
 }
 
 __device__ __forceinline__ void combine_out(int out_kind, double X, double Y, double Z, double (&o)[3]) {
@@ -130,15 +206,22 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
   }
   const double* yb = p.y + (size_t)b * 6 * p.N;
   double L[6];
-  orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
+  const double tn = fma((double)n, p.dt, p.t0);
+  if (!p.orb.nested) orbit_arm_times(p.orb, tn, L);
   double xyz[3];
   for (int c = 0; c < 3; ++c) {
     double acc = 0.0;
+    double tau[2][8];
+    if (p.orb.nested) {
+      chain_delays(p.orb, tn, p.path[c][0], tau[0]);
+      chain_delays(p.orb, tn, p.path[c][1], tau[1]);
+    }
     for (int s = 0; s < 4; ++s) {
       const K3Pair& pr = p.pair[c * 4 + s];
       const double* ser = yb + (size_t)pr.series * p.N;
       for (int k = 0; k < pr.n_terms; ++k) {
-        const double D = term_delay(pr.t[k], L, p.inv_dt);
+        const double D = p.orb.nested ? tau[(pr.t[k].chain >> 3) & 1][pr.t[k].chain & 7] * p.inv_dt
+                                      : term_delay(pr.t[k], L, p.inv_dt);
         const double Kf = ceil(D);
         const double eps = Kf - D;
         long long base = n - (long long)Kf;
@@ -272,7 +355,8 @@ struct K3Geom {
   static constexpr int CS = ((WIN + 2) / 8) * 8 + 5;  // odd, >= WIN, (CS-1) == 4 mod 8: conflict-free fragment reads
   static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
   static constexpr int CBUF = K3_PAIRS * K3_TS * CS;  // doubles of the stencil staging area
-  static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange
+  static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange (phase 1 with chained delays: [32][6][8] + [32][3][6])
+  static_assert(XBUF >= K3_TS * (48 + 18), "chained-delay scratch");
   // y buffer 0 is private (its first TMA copy overlaps the coefficient phase); the stencil
   // staging area shares its space with y buffer 1, which is first filled after phase 1
   static constexpr int UNION_PRIV = YBUF + (YBUF > CBUF ? YBUF : CBUF);
@@ -334,7 +418,31 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
   };
   if (G::PRIVATE0) prefetch(0, 0);  // chunk 0 lands in y buffer 0 while the coefficients are computed
   // ---- phase 1a: light travel times of the tile's samples
-  if (threadIdx.x < K3_TS) {
+  // (chained delays, A22: thread = (sample, channel, light path) walks its path leg by leg and
+  // parks the 8 delays in the X,Y,Z exchange area, which phase 2 has not touched yet)
+  double* taus = xs;  // [32][3][2][8]
+  if (p.orb.nested) {
+    double* Lq = taus + K3_TS * 6 * 8;  // [32][3][6]: KEPLER1 only
+    const double hq = 3.5 * p.orb.max_L;
+    if (p.orb.kind == 1) {
+      if (threadIdx.x < K3_TS * 3) {
+        const int sm = threadIdx.x % K3_TS, k = threadIdx.x / K3_TS;
+        double L[6];
+        orbit_arm_times(p.orb, fma((double)(n0 + sm), p.dt, p.t0) - (double)k * hq, L);
+#pragma unroll
+        for (int l = 0; l < 6; ++l) Lq[(sm * 3 + k) * 6 + l] = L[l];
+      }
+      __syncthreads();
+    }
+    if (threadIdx.x < K3_TS * 6) {
+      const int sm = threadIdx.x % K3_TS, cp = threadIdx.x / K3_TS;  // cp = channel * 2 + path
+      double tau[8];
+      if (p.orb.kind == 1) chain_delays_quad(Lq + sm * 18, 1.0 / hq, p.path[cp >> 1][cp & 1], tau);
+      else chain_delays(p.orb, fma((double)(n0 + sm), p.dt, p.t0), p.path[cp >> 1][cp & 1], tau);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) taus[(sm * 6 + cp) * 8 + i] = tau[i];
+    }
+  } else if (threadIdx.x < K3_TS) {
     double L[6];
     orbit_arm_times(p.orb, fma((double)(n0 + threadIdx.x), p.dt, p.t0), L);
 #pragma unroll
@@ -354,7 +462,9 @@ __global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
 #pragma unroll
       for (int l = 0; l < 6; ++l) L[l] = Ls[sm * 6 + l];
       for (int k = 0; k < pr.n_terms; ++k) {
-        const double D = term_delay(pr.t[k], L, p.inv_dt);
+        const int chn = pr.t[k].chain;
+        const double D = p.orb.nested ? taus[(sm * 6 + (pi / 4) * 2 + ((chn >> 3) & 1)) * 8 + (chn & 7)] * p.inv_dt
+                                      : term_delay(pr.t[k], L, p.inv_dt);
         const double Kf = ceil(D);
         const double eps = Kf - D;
         int off = KCAP - (int)Kf;
@@ -505,7 +615,8 @@ int run_tdi(int B, long long N, double t0, double dt, int order, int generation,
   p.margin_lo = margin_lo; p.margin_hi = margin_hi; p.y = y; p.tdi = tdi; p.orb = orb;
   make_lagw(order, &p.lw);
   make_lags(order, &p.ls);
-  build_pairs(generation, p.pair);
+  if (build_pairs(generation, p.pair, p.path))
+    return set_error(LISA_TD_EINVAL, "tdi: internal term table does not match the light paths");
   const int nL = generation == 20 ? 7 : 3;
   const int kcap = (int)ceil(nL * orb.max_L / dt);
   p.kcap = kcap;

@@ -39,7 +39,7 @@ class Orbit(C.Structure):
     _fields_ = [("kind", C.c_int), ("L_m", C.c_double), ("a_m", C.c_double),
                 ("year_s", C.c_double), ("phase0", C.c_double), ("t_ref", C.c_double),
                 ("r_static", (C.c_double * 3) * 3), ("L_static", C.c_double * 6),
-                ("table", C.c_void_p)]
+                ("table", C.c_void_p), ("tt_order", C.c_int), ("tdi_nested", C.c_int)]
 
 
 class OrbitTable:
@@ -86,6 +86,8 @@ def make_orbit(d: dict) -> Orbit:
         o.table = d["_lisa_table"]._h
     else:
         raise ValueError(d["kind"])
+    o.tt_order = int(d.get("tt_order", 0))  # delay model, reading A22
+    o.tdi_nested = int(d.get("nested", 0))
     return o
 
 

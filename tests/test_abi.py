@@ -34,8 +34,9 @@ def test_version_and_error_string(lib):
 
 
 def test_orbit_struct_layout_matches_header(lib):
-    # int + pad, 5 doubles, 9 doubles, 6 doubles, one pointer
-    assert C.sizeof(lib.Orbit) == 8 + 5 * 8 + 9 * 8 + 6 * 8 + 8
+    # int + pad, 5 doubles, 9 doubles, 6 doubles, one pointer, two ints (delay model, reading A22)
+    assert C.sizeof(lib.Orbit) == 8 + 5 * 8 + 9 * 8 + 6 * 8 + 8 + 8
+    assert lib.Orbit.tt_order.offset == 176 and lib.Orbit.tdi_nested.offset == 180
 
 
 def test_argument_validation_happens_before_any_launch(lib):
@@ -55,6 +56,11 @@ def test_argument_validation_happens_before_any_launch(lib):
     # margin too small for the orbit: |k.r|/c can reach ~500 s = 100 samples
     rc = L.lisa_td_link_response(1, 4096, 0.0, 5.0, 31, 64, fake, fake, fake, fake, C.byref(orb), fake, None)
     assert rc == -1 and "margin_y" in lib.last_error()
+    # delay model flags outside {0, 1}
+    bad = lib.make_orbit({"kind": "kepler1", "L_m": 2.5e9, "a_m": 1.495978707e11, "year_s": 365.25 * 86400,
+                          "tt_order": 2})
+    rc = L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 20, 1, 160, 144, fake, C.byref(bad), fake, None)
+    assert rc == -1 and "tt_order" in lib.last_error()
     # TDI: bad generation, small margins
     assert L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 17, 1, 160, 144, fake, C.byref(orb), fake, None) == -1
     assert L.lisa_td_tdi2(1, 4096, 0.0, 5.0, 31, 20, 1, 20, 144, fake, C.byref(orb), fake, None) == -1
