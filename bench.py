@@ -338,6 +338,18 @@ def run_ours(args):
                 "ms_s1_plus_s2_full_rate": stage_ms["S1_modes_to_pol"] + stage_ms["S2_link_response"],
                 "cite": "PAPER.md:243 (10 s sampling, linear interpolation), DESIGN.md reading A20"}
     del c_in, hpc, hcc
+    # ---- SURVEY 8(f) f4, second half: channel subsets A / AE: S4 + S5 on fewer channels
+    ch_info = {"ms_s45_AET": stage_ms["S45_fft_loglike"], "cite": "PAPER.md:362"}
+    for n_ch, name in ((1, "ms_s45_A"), (2, "ms_s45_AE")):
+        for _ in range(3):
+            lib.loglike_channels(plan, B, N, n_ch, tdi, data, weight, kmin, kmax, ll, dh, hh)
+        ce = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ce[0].record()
+        for _ in range(5):
+            lib.loglike_channels(plan, B, N, n_ch, tdi, data, weight, kmin, kmax, ll, dh, hh)
+        ce[1].record()
+        torch.cuda.synchronize()
+        ch_info[name] = ce[0].elapsed_time(ce[1]) / 5
     # ---- first-order light travel times + TDI delays chained along the light path
     # (reading A22): S2 and S3 with that delay model (restores y, tdi of the default model after)
     orb22 = dict(inp["orbit"], tt_order=1, nested=1)
@@ -435,7 +447,7 @@ def run_ours(args):
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
-        "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info},
+        "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info},
     }
     print(json.dumps(line))
     plan.close()

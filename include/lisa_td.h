@@ -174,6 +174,14 @@ LISA_TD_API int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const do
                     const double* data_spec, const double* weight, long long kmin, long long kmax,
                     double* loglike, double* dh, double* hh, void* stream);
 
+/* The same with a subset of the channels ("injections and recoveries were performed
+ * using one (A), two (AE) and three (AET) TDI channels"): the sums over c run over the first
+ * n_channels (1, 2 or 3) of A,E,T; the other channels of tdi are neither transformed nor read.
+ * Layouts as above (tdi stays [B][3][N], data_spec and weight stay [3][...]). */
+LISA_TD_API int lisa_td_loglike_channels(lisa_td_plan* plan, int B, long long N, int n_channels, const double* tdi,
+                             const double* data_spec, const double* weight, long long kmin, long long kmax,
+                             double* loglike, double* dh, double* hh, void* stream);
+
 /* Fisher matrix by first-order finite differences ("The Fisher matrix is computed
  * from the derivatives of the likelihood function, using first-order finite differences";
  * reading A19 of DESIGN.md).  tdi: [D+1][3][N] (A,E,T): walker 0 is the centre theta, walker

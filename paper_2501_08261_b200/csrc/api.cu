@@ -223,7 +223,7 @@ int plan_create(Plan**, int, long long);
 int plan_destroy(Plan*);
 int run_spectrum(Plan*, int, long long, const double*, double*, cudaStream_t);
 int run_loglike(Plan*, int, long long, const double*, const double*, const double*, long long,
-                long long, double*, double*, double*, cudaStream_t);
+                long long, double*, double*, double*, cudaStream_t, int n_ch);
 int run_fisher(Plan*, int, long long, const double*, const double*, const double*, long long, long long,
                double*, cudaStream_t);
 extern int g_force_generic;
@@ -494,7 +494,22 @@ int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const double* tdi,
   int rc = check_band(fn, N, kmin, kmax);
   if (rc) return rc;
   REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, data_spec); REQUIRE_PTR(fn, weight); REQUIRE_PTR(fn, loglike);
-  return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream);
+  return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream, 3);
+}
+
+int lisa_td_loglike_channels(lisa_td_plan* plan, int B, long long N, int n_channels, const double* tdi,
+                             const double* data_spec, const double* weight, long long kmin, long long kmax,
+                             double* loglike, double* dh, double* hh, void* stream) {
+  const char* fn = "lisa_td_loglike_channels";
+  if (!plan) return set_error(LISA_TD_EINVAL, "%s: plan is NULL", fn);
+  if (B <= 0) return set_error(LISA_TD_EINVAL, "%s: B must be > 0", fn);
+  if (n_channels < 1 || n_channels > 3)
+    return set_error(LISA_TD_EINVAL, "%s: n_channels=%d must be 1 (A), 2 (A,E) or 3 (A,E,T)", fn, n_channels);
+  int rc = check_band(fn, N, kmin, kmax);
+  if (rc) return rc;
+  REQUIRE_PTR(fn, tdi); REQUIRE_PTR(fn, data_spec); REQUIRE_PTR(fn, weight); REQUIRE_PTR(fn, loglike);
+  return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream,
+                     n_channels);
 }
 
 int lisa_td_fisher(lisa_td_plan* plan, int D, long long N, const double* tdi, const double* delta_host,
@@ -686,7 +701,7 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
     if ((rc = run_tdi((int)nb, N, t0, dt, order, generation, 1, margin_lo, margin_hi, p->y, od, p->tdi, p->s_comp)))
       return rc;
     if ((rc = run_loglike(p->plan, (int)nb, N, p->tdi, p->data_spec, p->weight, kmin, kmax, p->ll, p->ll + sc_stride,
-                          p->ll + 2 * sc_stride, p->s_comp)))
+                          p->ll + 2 * sc_stride, p->s_comp, 3)))
       return rc;
     LISA_CUDA(cudaMemcpyAsync(loglike_host + b0, p->ll, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));
     if (dh_host) LISA_CUDA(cudaMemcpyAsync(dh_host + b0, p->ll + sc_stride, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));

@@ -61,7 +61,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 __global__ void __launch_bounds__(K5_THREADS) k5_inner_partial(
     const double2* __restrict__ spec, const double2* __restrict__ data,
     const double* __restrict__ weight, long long nf, long long kmin, long long kmax,
-    double two_pi_over_N, double2* __restrict__ partial) {
+    double two_pi_over_N, double2* __restrict__ partial, int n_ch) {
   const int b = blockIdx.y, slice = blockIdx.x;
   const long long nk = kmax - kmin + 1;
   const long long per = (nk + K5_SLICES - 1) / K5_SLICES;
@@ -74,6 +74,7 @@ __global__ void __launch_bounds__(K5_THREADS) k5_inner_partial(
     bin_twiddle(k, two_pi_over_N, cw, sw);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
+      if (c >= n_ch) break;  // channel subset A / A,E / A,E,T
       const double2 h = packed_bin(spec + ((size_t)b * 3 + c) * M, M, k, cw, sw);
       const double2 d = data[(size_t)c * nf + k];
       const double w = weight[(size_t)c * nf + k];
@@ -201,8 +202,11 @@ static int check_fft(cufftResult r, const char* what) {
   return set_error(LISA_TD_ECUDA, "%s failed: cufftResult %d", what, (int)r);
 }
 
-static int get_fft(Plan* pl, int B, cufftHandle* h) {
-  auto it = pl->fft.find(B);
+// single != 0: one channel per walker (input and output strides of three rows), executed once
+// per selected channel; otherwise all 3B rows in one batch.
+static int get_fft(Plan* pl, int B, cufftHandle* h, int single = 0) {
+  const int key = 2 * B + (single ? 1 : 0);
+  auto it = pl->fft.find(key);
   if (it != pl->fft.end()) {
     *h = it->second;
     return LISA_TD_OK;
@@ -212,13 +216,15 @@ static int get_fft(Plan* pl, int B, cufftHandle* h) {
   if (rc != LISA_TD_OK) return rc;
   long long n[1] = {pl->N / 2};
   size_t ws = 0;
-  rc = check_fft(cufftMakePlanMany64(f, 1, n, nullptr, 1, pl->N / 2, nullptr, 1, pl->N / 2, CUFFT_Z2Z, 3LL * B, &ws),
+  long long embed[1] = {pl->N / 2};
+  const long long dist = single ? 3 * (pl->N / 2) : pl->N / 2;
+  rc = check_fft(cufftMakePlanMany64(f, 1, n, embed, 1, dist, embed, 1, dist, CUFFT_Z2Z, single ? (long long)B : 3LL * B, &ws),
                  "cufftMakePlanMany64");
   if (rc != LISA_TD_OK) {
     cufftDestroy(f);
     return rc;
   }
-  pl->fft[B] = f;
+  pl->fft[key] = f;
   *h = f;
   return LISA_TD_OK;
 }
@@ -252,13 +258,22 @@ int plan_destroy(Plan* pl) {
 
 // FFT of B <= capacity walkers.  A plan for a batch size not seen before is created on first
 // use (that call synchronises inside cuFFT).
-static int run_fft(Plan* pl, int B, const double* tdi, double2* spec, cudaStream_t st) {
+static int run_fft(Plan* pl, int B, const double* tdi, double2* spec, cudaStream_t st, int n_ch = 3) {
   if (B > pl->B) return set_error(LISA_TD_EINVAL, "B=%d exceeds the plan's capacity %d", B, pl->B);
   cufftHandle h;
-  int rc = get_fft(pl, B, &h);
+  int rc = get_fft(pl, B, &h, n_ch < 3);
   if (rc != LISA_TD_OK) return rc;
   rc = check_fft(cufftSetStream(h, st), "cufftSetStream");
   if (rc != LISA_TD_OK) return rc;
+  if (n_ch < 3) {  // only the selected channels are transformed
+    for (int c = 0; c < n_ch; ++c) {
+      rc = check_fft(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(const_cast<double*>(tdi)) + (size_t)c * (pl->N / 2),
+                                  reinterpret_cast<cufftDoubleComplex*>(spec) + (size_t)c * (pl->N / 2), CUFFT_FORWARD),
+                     "cufftExecZ2Z");
+      if (rc != LISA_TD_OK) return rc;
+    }
+    return LISA_TD_OK;
+  }
   return check_fft(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(const_cast<double*>(tdi)),
                                 reinterpret_cast<cufftDoubleComplex*>(spec), CUFFT_FORWARD),
                    "cufftExecZ2Z");
@@ -287,13 +302,13 @@ int run_spectrum(Plan* pl, int B, long long N, const double* tdi, double* spec, 
 
 int run_loglike(Plan* pl, int B, long long N, const double* tdi, const double* data_spec,
                 const double* weight, long long kmin, long long kmax, double* loglike, double* dh,
-                double* hh, cudaStream_t st) {
+                double* hh, cudaStream_t st, int n_ch) {
   if (N != pl->N) return set_error(LISA_TD_EINVAL, "loglike: N differs from the plan's");
-  int rc = run_fft(pl, B, tdi, pl->spec, st);
+  int rc = run_fft(pl, B, tdi, pl->spec, st, n_ch);
   if (rc != LISA_TD_OK) return rc;
   dim3 grid(K5_SLICES, (unsigned)B);
   k5_inner_partial<<<grid, K5_THREADS, 0, st>>>(pl->spec, reinterpret_cast<const double2*>(data_spec), weight,
-                                                pl->nf, kmin, kmax, 6.283185307179586476925 / (double)N, pl->partial);
+                                                pl->nf, kmin, kmax, 6.283185307179586476925 / (double)N, pl->partial, n_ch);
   LISA_LAUNCH_CHECK("k5_inner_partial");
   k5_inner_final<<<(B + 127) / 128, 128, 0, st>>>(pl->partial, B, loglike, dh, hh);
   LISA_LAUNCH_CHECK("k5_inner_final");

@@ -22,6 +22,7 @@ EXPORTS = [
     "lisa_td_link_response_up2",
     "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_response_tdi_workspace_bytes",
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
+    "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
     "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_probe_dfma",
     "lisa_td_debug_force_generic",
@@ -121,6 +122,7 @@ def load() -> C.CDLL:
     L.lisa_td_plan_create.argtypes = [C.POINTER(vp), i32, i64]
     L.lisa_td_plan_destroy.argtypes = [vp]
     L.lisa_td_loglike.argtypes = [vp, i32, i64, vp, vp, vp, i64, i64, vp, vp, vp, vp]
+    L.lisa_td_loglike_channels.argtypes = [vp, i32, i64, i32, vp, vp, vp, i64, i64, vp, vp, vp, vp]
     L.lisa_td_spectrum.argtypes = [vp, i32, i64, vp, vp, vp]
     L.lisa_td_fisher.argtypes = [vp, i32, i64, vp, vp, vp, i64, i64, vp, vp]
     L.lisa_td_psd_weights.argtypes = [i64, dbl, dbl, dbl, dbl, i32, vp]
@@ -249,6 +251,11 @@ class Plan:
 def loglike(plan: Plan, B, N, tdi, data_spec, weight, kmin, kmax, loglike_out, dh=None, hh=None):
     _check(load().lisa_td_loglike(plan._h, B, N, _dev(tdi), _dev(data_spec), _dev(weight), kmin, kmax,
                                   _dev(loglike_out), _dev(dh), _dev(hh), _stream()))
+
+
+def loglike_channels(plan: Plan, B, N, n_channels, tdi, data_spec, weight, kmin, kmax, loglike_out, dh=None, hh=None):
+    _check(load().lisa_td_loglike_channels(plan._h, B, N, int(n_channels), _dev(tdi), _dev(data_spec), _dev(weight),
+                                           kmin, kmax, _dev(loglike_out), _dev(dh), _dev(hh), _stream()))
 
 
 def spectrum(plan: Plan, B, N, tdi, spec):
