@@ -373,6 +373,28 @@ def run_ours(args):
     nested_info = {"ms_s2_tt_order1": ne[0].elapsed_time(ne[1]) / 5, "ms_s3_chained": ne[1].elapsed_time(ne[2]) / 5,
                    "ms_s2_default": stage_ms["S2_link_response"], "ms_s3_default": stage_ms["S3_tdi2"],
                    "cite": "PAPER.md:163, 380-384; DESIGN.md reading A22"}
+    # ---- "with p = 1 (the paper's linear interpolation) also timed"
+    def o1_s2():
+        lib.link_response(B, N, t0, dt, 1, inp["margin_y"], hp, hc, g("lam"), g("beta_sky"), inp["orbit"], y)
+
+    def o1_s3():
+        lib.tdi2(B, N, t0, dt, 1, 20, 1, inp["margin_lo"], inp["margin_hi"], y, inp["orbit"], tdi)
+    for _ in range(3):
+        o1_s2(); o1_s3()
+    oe = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    oe[0].record()
+    for _ in range(5):
+        o1_s2()
+    oe[1].record()
+    for _ in range(5):
+        o1_s3()
+    oe[2].record()
+    torch.cuda.synchronize()
+    o1_ms2, o1_ms3 = oe[0].elapsed_time(oe[1]) / 5, oe[1].elapsed_time(oe[2]) / 5
+    order1_info = {"ms_s2": o1_ms2, "ms_s3": o1_ms3,
+                   "s2_hbm_gbs": 64.0 * B * N / (o1_ms2 * 1e-3) / 1e9, "s3_hbm_gbs": 72.0 * B * N / (o1_ms3 * 1e-3) / 1e9,
+                   "hbm_bytes_per_walker_sample": {"s2": 64, "s3": 72},
+                   "cite": "PAPER.md:209 (linear interpolation); SURVEY 8(d)"}
     s2(); s3()
     torch.cuda.synchronize()
     fisher_info = {"D": D, "walkers": D + 1, "ms_per_matrix": fe[0].elapsed_time(fe[1]) / 5,
@@ -447,7 +469,8 @@ def run_ours(args):
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
-        "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info},
+        "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info,
+                 "order1": order1_info},
     }
     print(json.dumps(line))
     plan.close()

@@ -165,6 +165,15 @@ static int make_orbit_dev_kind(const lisa_td_orbit* o, OrbitDev* d) {
   if (o->kind != 1) return set_error(LISA_TD_EINVAL, "orbit: unknown kind %d", o->kind);
   if (!(o->a_m > 0) || !(o->L_m > 0) || !(o->year_s > 0))
     return set_error(LISA_TD_EINVAL, "orbit: KEPLER1 needs a_m, L_m, year_s > 0");
+  // the bounds below take ~3 ms of long-double libm per evaluation: remember the last orbit of
+  // this thread (a sampler calls with the same orbit millions of times)
+  struct Memo { bool valid; double key[5]; OrbitDev dev; };
+  static thread_local Memo memo = {false, {0, 0, 0, 0, 0}, {}};
+  const double key[5] = {o->L_m, o->a_m, o->year_s, o->phase0, o->t_ref};
+  if (memo.valid && memcmp(memo.key, key, sizeof(key)) == 0) {
+    *d = memo.dev;
+    return LISA_TD_OK;
+  }
   const long double PI_L = 3.14159265358979323846264338327950288L;
   long double a = o->a_m, delta = (long double)o->L_m / (2 * a), sq3 = sqrtl(3.0L);
   long double e = sqrtl(1 + 2 * delta / sq3 + 4 * delta * delta / 3) - 1;
@@ -205,6 +214,9 @@ static int make_orbit_dev_kind(const lisa_td_orbit* o, OrbitDev* d) {
   d->max_L = (double)(mL * 1.001L / C_LIGHT);
   d->max_off_over_c = (double)(mo * 1.001L / C_LIGHT);
   d->max_dc_rate = d->a_over_c * d->w;
+  memcpy(memo.key, key, sizeof(key));
+  memo.dev = *d;
+  memo.valid = true;
   return LISA_TD_OK;
 }
 
