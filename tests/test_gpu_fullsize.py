@@ -139,6 +139,57 @@ def test_config4_full_size_loglike(lib, orc_d):
     plan.close()
 
 
+def test_config2_full_size_single_source(lib, orc):
+    """configs[1]: one source, N = 2^20, aligned spin (no Euler angles), KEPLER1, TDI-2 A,E,T:
+    the whole series against the long-double oracle (the batch-1 launch configuration)."""
+    B, N = 1, 1 << 20
+    inp = synth.make_inputs(2, device="cuda", B=B, N=N)
+    assert inp["alpha"] is None
+    _, _, _, tdi = _gpu_chain_full(lib, inp, B, N)
+    h = _walker_to_host(inp, 0)
+    ref = _orc_window(orc, inp, h, 0, N, want=("tdi",))["tdi"][0]
+    got = tdi[0].cpu().numpy()
+    common = max(np.linalg.norm(ref[c]) for c in range(3))
+    raw = [float(np.linalg.norm(got[c] - ref[c]) / np.linalg.norm(ref[c])) for c in range(3)]
+    com = [float(np.linalg.norm(got[c] - ref[c]) / common) for c in range(3)]
+    print(f"config 2 full length: raw rel-L2 {raw}, vs common scale {com}")
+    assert raw[0] < TOL_TDI and raw[1] < TOL_TDI
+    assert com[2] < TOL_TDI and raw[2] < 1e-8
+
+
+def test_config4_batch_256(lib, orc_d):
+    """configs[3] as stated: batch 256 in ONE launch per stage (48 GiB of arrays on the device);
+    log L of the first, a middle and the last walker against the oracle's own chain."""
+    B, N = 256, 1 << 20
+    inp = synth.make_inputs(4, device="cuda", B=B, N=N)
+    dt = inp["dt"]
+    kmin, kmax = synth.likelihood_band(N, dt)
+    hp, hc, y, tdi = _gpu_chain_full(lib, inp, B, N)
+    del hp, hc, y
+    plan = lib.Plan(B, N)
+    spec = torch.empty((1, 3, N // 2 + 1, 2), dtype=torch.float64, device="cuda")
+    lib.spectrum(plan, 1, N, tdi[:1], spec)
+    data_gpu = spec[0].contiguous()
+    w_gpu = torch.from_numpy(lib.psd_weights(N, dt, synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)).cuda()
+    ll, dh, hh = (torch.empty(B, dtype=torch.float64, device="cuda") for _ in range(3))
+    lib.loglike(plan, B, N, tdi, data_gpu, w_gpu, kmin, kmax, ll, dh, hh)
+    torch.cuda.synchronize()
+    assert torch.isfinite(ll).all()
+    w = orc_d.psd_weights(N, dt, synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)
+    h0 = _walker_to_host(inp, 0)
+    data = orc_d.spectrum3(_orc_window(orc_d, inp, h0, 0, N, want=("tdi",))["tdi"][0])
+    for b in (0, 131, 255):
+        hb = _walker_to_host(inp, b)
+        ref = _orc_window(orc_d, inp, hb, 0, N, want=("loglike",), data_spec=data, weight=w, kmin=kmin, kmax=kmax)
+        for got, key in ((ll, "loglike"), (dh, "dh"), (hh, "hh")):
+            err = abs(got[b].item() - ref[key][0]) / abs(ref[key][0])
+            print(b, key, err)
+            assert err < TOL_LL, (b, key, err)
+    plan.close()
+    del tdi, inp
+    torch.cuda.empty_cache()
+
+
 def test_config5_stress_sampled(lib, orc, orc_d):
     """configs[4]: N = 2^22, B = 32, precessing, Kepler arms; plus the common laser-noise stream
     through the link helper and TDI-2 at full length (reading A12, P6: absolute tolerance)."""
