@@ -69,6 +69,43 @@ __device__ __forceinline__ void read_pair2(const double2* __restrict__ xe, const
   }
 }
 
+// Walker-independent geometry of the thread's two samples na, na + 1 -> geo[field][sample]
+// (fields: 0,1,20 common delay per unit k; 2..10 spacecraft offsets as delays per unit k;
+// 11..13 / 14..16 light travel times of links +a / -a; 17..19 reciprocal arm lengths; samples).
+template <int KIND>
+__device__ __forceinline__ void k2_geometry(const K2Params& p, double* geo, long long na) {
+#pragma unroll 1
+  for (int c = 0; c < 2; ++c) {
+    double* gq = geo + 2 * threadIdx.x + c;
+    double d[3][3], rc_s[3], vel[3][3];
+    if (p.orb.tt_order) orbit_offsets_v<true>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
+    else orbit_offsets_v<false>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
+    const double sc = p.inv_dt / C_LIGHT;
+    gq[0 * K2_T] = rc_s[0] * p.inv_dt;   // common (1 AU) delay per unit k (samples)
+    gq[1 * K2_T] = rc_s[1] * p.inv_dt;
+    gq[20 * K2_T] = rc_s[2] * p.inv_dt;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) gq[(2 + 3 * k + j) * K2_T] = d[k][j] * sc;  // offsets as delays per unit k
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const int s = link_s(a), r = link_r(a);
+      const double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
+      const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) * sc;  // arm length in samples
+      double Lp = len, Lm = len;  // light travel times of links +a, -a (KEPLER1, TABLE: |r_r - r_s|/c)
+      if (KIND != 0 && p.orb.tt_order) {  // A22: (d/c)(1 + n.v_sender/c); link -a runs r -> s
+        const double q = sc / (len * C_LIGHT);  // n.v/c = (d.v) q with d in metres, len in samples
+        Lp = fma(len, fma(dx, vel[s][0], fma(dy, vel[s][1], dz * vel[s][2])) * q, len);
+        Lm = fma(len, -fma(dx, vel[r][0], fma(dy, vel[r][1], dz * vel[r][2])) * q, len);
+      }
+      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : Lp;
+      gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : Lm;
+      gq[(17 + a) * K2_T] = 1.0 / len;  // n_a = (offset_r - offset_s) / len
+    }
+  }
+}
+
 template <int HT, int KIND>
 __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params p) {
   extern __shared__ double2 smem2[];  // [2 buffers][even, odd][LE] strain tiles, then geo[K2_NGEO][K2_T]
@@ -142,36 +179,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 
   // ---- walker-independent geometry of this thread's two samples -> geo[field][sample]
   const long long na = n0 + 2 * threadIdx.x;
-#pragma unroll 1
-  for (int c = 0; c < 2; ++c) {
-    double* gq = geo + 2 * threadIdx.x + c;
-    double d[3][3], rc_s[3], vel[3][3];
-    if (p.orb.tt_order) orbit_offsets_v<true>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
-    else orbit_offsets_v<false>(p.orb, fma((double)(na + c), p.dt, p.t0), d, rc_s, vel);
-    const double sc = p.inv_dt / C_LIGHT;
-    gq[0 * K2_T] = rc_s[0] * p.inv_dt;   // common (1 AU) delay per unit k (samples)
-    gq[1 * K2_T] = rc_s[1] * p.inv_dt;
-    gq[20 * K2_T] = rc_s[2] * p.inv_dt;
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-#pragma unroll
-      for (int j = 0; j < 3; ++j) gq[(2 + 3 * k + j) * K2_T] = d[k][j] * sc;  // offsets as delays per unit k
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      const int s = link_s(a), r = link_r(a);
-      const double dx = d[r][0] - d[s][0], dy = d[r][1] - d[s][1], dz = d[r][2] - d[s][2];
-      const double len = sqrt(fma(dx, dx, fma(dy, dy, dz * dz))) * sc;  // arm length in samples
-      double Lp = len, Lm = len;  // light travel times of links +a, -a (KEPLER1, TABLE: |r_r - r_s|/c)
-      if (KIND != 0 && p.orb.tt_order) {  // A22: (d/c)(1 + n.v_sender/c); link -a runs r -> s
-        const double q = sc / (len * C_LIGHT);  // n.v/c = (d.v) q with d in metres, len in samples
-        Lp = fma(len, fma(dx, vel[s][0], fma(dy, vel[s][1], dz * vel[s][2])) * q, len);
-        Lm = fma(len, -fma(dx, vel[r][0], fma(dy, vel[r][1], dz * vel[r][2])) * q, len);
-      }
-      gq[(11 + a) * K2_T] = KIND == 0 ? p.orb.L[a] * p.inv_dt : Lp;
-      gq[(14 + a) * K2_T] = KIND == 0 ? p.orb.L[a + 3] * p.inv_dt : Lm;
-      gq[(17 + a) * K2_T] = 1.0 / len;  // n_a = (offset_r - offset_s) / len
-    }
-  }
+  k2_geometry<KIND>(p, geo, na);
   const bool act[2] = {na >= R && na < p.N - R, na + 1 >= R && na + 1 < p.N - R};
   const bool vec_store = (p.N & 1) == 0;
   const int elo = p.half - 1, ehi = tile_len - 2 - p.half;
@@ -282,6 +290,150 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 #undef GEO2
 }
 
+// ---------------------------------------------------------------- linear interpolation (p = 1)
+// The paper's own GPU code interpolates linearly.  With two taps per read there
+// is nothing to stage: each thread reads its taps straight from global memory (adjacent
+// threads read adjacent samples; the nine reads of a walker fall within ~100 samples, so they
+// hit L1), the walker loop has no barrier, all nine reads are unrolled, and a block serves up
+// to K2L_G walkers with one evaluation of the orbit geometry.
+constexpr int K2L_G = 32;
+
+__device__ __forceinline__ void read_pair_lin(const double* __restrict__ hp, const double* __restrict__ hc,
+                                              long long na, long long N, const double (&Dc)[2], double Dla,
+                                              double Dlb, double (&vp)[2], double (&vc)[2]) {
+  const double Ka = ceil(Dc[0] + Dla), Kb = ceil(Dc[1] + Dlb);
+  const double epsa = (Ka - Dc[0]) - Dla, epsb = (Kb - Dc[1]) - Dlb;
+  // taps j = 0, 1: x[n - K], x[n - K + 1] with weights 1 - eps, eps (clamped for memory safety
+  // only: margin_y keeps every window inside [0, N))
+  const long long ia = max(0LL, min(na - (long long)Ka, N - 2));
+  const long long ib = max(0LL, min(na + 1 - (long long)Kb, N - 2));
+  const double a0 = __ldg(hp + ia), a1 = __ldg(hp + ia + 1);
+  const double c0 = __ldg(hc + ia), c1 = __ldg(hc + ia + 1);
+  const bool shared_tap = ib == ia + 1;  // same integer delay: sample b starts on a's second tap
+  const double b0 = shared_tap ? a1 : __ldg(hp + ib), d0 = shared_tap ? c1 : __ldg(hc + ib);
+  const double b1 = __ldg(hp + ib + 1), d1 = __ldg(hc + ib + 1);
+  vp[0] = fma(epsa, a1 - a0, a0);
+  vc[0] = fma(epsa, c1 - c0, c0);
+  vp[1] = fma(epsb, b1 - b0, b0);
+  vc[1] = fma(epsb, d1 - d0, d0);
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response_lin(const K2Params p) {
+  extern __shared__ double geo[];    // [K2_NGEO][K2_T]; a thread only ever reads its own two samples
+  __shared__ double sky[K2L_G][9];   // k, u, v of the block's walkers (Eq. 2.7)
+  const int R = p.margin;
+  const long long n0 = (long long)blockIdx.x * K2_T;
+  const int w0 = blockIdx.y * p.group;
+  const int nw = min(p.group, p.B - w0);
+#define GEO2(f) (*reinterpret_cast<const double2*>(geo + (f) * K2_T + 2 * threadIdx.x))
+  if (threadIdx.x < nw) {
+    double sl, cl, sb, cb;
+    sincos_d(p.lambda[w0 + threadIdx.x], sl, cl);
+    sincos_d(p.beta_sky[w0 + threadIdx.x], sb, cb);
+    double* s = sky[threadIdx.x];
+    s[0] = -cb * cl; s[1] = -cb * sl; s[2] = -sb;  // k
+    s[3] = sl;       s[4] = -cl;      s[5] = 0.0;  // u
+    s[6] = -sb * cl; s[7] = -sb * sl; s[8] = cb;   // v
+  }
+  const long long na = n0 + 2 * threadIdx.x;
+  k2_geometry<KIND>(p, geo, na);
+  __syncthreads();
+  const bool act[2] = {na >= R && na < p.N - R, na + 1 >= R && na + 1 < p.N - R};
+  const bool vec_store = (p.N & 1) == 0;
+  if (na >= p.N) return;
+
+  for (int w = 0; w < nw; ++w) {
+    const double* hp = p.hplus + (size_t)(w0 + w) * p.N;
+    const double* hc = p.hcross + (size_t)(w0 + w) * p.N;
+    double* yb = p.y + (size_t)(w0 + w) * 6 * p.N + na;
+    auto store2 = [&](int l, double v0, double v1) {
+      double* dst = yb + (size_t)l * p.N;
+      v0 = act[0] ? v0 : 0.0;
+      v1 = act[1] ? v1 : 0.0;
+      if (vec_store) {
+        *reinterpret_cast<double2*>(dst) = make_double2(v0, v1);
+      } else {
+        dst[0] = v0;
+        if (na + 1 < p.N) dst[1] = v1;
+      }
+    };
+    if (!(act[0] || act[1])) {
+#pragma unroll
+      for (int l = 0; l < 6; ++l) store2(l, 0.0, 0.0);
+      continue;
+    }
+    const double* s = sky[w];
+    const double kx = s[0], ky = s[1], kz = s[2];
+    const double ux = s[3], uy = s[4];  // uz = 0
+    const double vx = s[6], vy = s[7], vz = s[8];
+    double Dc[2];
+    {
+      const double2 g0 = GEO2(0), g1 = GEO2(1);
+      Dc[0] = fma(kx, g0.x, ky * g1.x);
+      Dc[1] = fma(kx, g0.y, ky * g1.y);
+      if (KIND == 2) {
+        const double2 g2 = GEO2(20);
+        Dc[0] = fma(kz, g2.x, Dc[0]);
+        Dc[1] = fma(kz, g2.y, Dc[1]);
+      }
+    }
+    double kd[3][2], ud[3][2], vd[3][2], hpr[3][2], hcr[3][2];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const double2 dx = GEO2(2 + 3 * k), dy = GEO2(3 + 3 * k), dz = GEO2(4 + 3 * k);
+      kd[k][0] = fma(kx, dx.x, fma(ky, dy.x, kz * dz.x));
+      kd[k][1] = fma(kx, dx.y, fma(ky, dy.y, kz * dz.y));
+      ud[k][0] = fma(ux, dx.x, uy * dy.x);
+      ud[k][1] = fma(ux, dx.y, uy * dy.y);
+      vd[k][0] = fma(vx, dx.x, fma(vy, dy.x, vz * dz.x));
+      vd[k][1] = fma(vx, dx.y, fma(vy, dy.y, vz * dz.y));
+      read_pair_lin(hp, hc, na, p.N, Dc, kd[k][0], kd[k][1], hpr[k], hcr[k]);  // h(t - k.r_k/c)
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {  // links a and -a share x+, xx and have opposite n
+      const int sd = link_s(a), rc = link_r(a);
+      const double2 Lp = GEO2(11 + a), Lm = GEO2(14 + a), il = GEO2(17 + a);
+      const double ila[2] = {il.x, il.y};
+      double xp[2], xc2[2], fp[2], fm[2];
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const double un = (ud[rc][c] - ud[sd][c]) * ila[c];
+        const double vn = (vd[rc][c] - vd[sd][c]) * ila[c];
+        const double kn = (kd[rc][c] - kd[sd][c]) * ila[c];
+        xp[c] = fma(un, un, -vn * vn);
+        xc2[c] = 2.0 * un * vn;
+        const double om = 1.0 - kn, opl = 1.0 + kn;
+        const double inv = 0.5 / (om * opl);
+        fp[c] = opl * inv;
+        fm[c] = om * inv;
+      }
+      double hps[2], hcs[2];
+      read_pair_lin(hp, hc, na, p.N, Dc, Lp.x + kd[sd][0], Lp.y + kd[sd][1], hps, hcs);  // link +a: s -> r
+      store2(a, fma(xp[0], hps[0] - hpr[rc][0], xc2[0] * (hcs[0] - hcr[rc][0])) * fp[0],
+             fma(xp[1], hps[1] - hpr[rc][1], xc2[1] * (hcs[1] - hcr[rc][1])) * fp[1]);
+      read_pair_lin(hp, hc, na, p.N, Dc, Lm.x + kd[rc][0], Lm.y + kd[rc][1], hps, hcs);  // link -a: r -> s
+      store2(a + 3, fma(xp[0], hps[0] - hpr[sd][0], xc2[0] * (hcs[0] - hcr[sd][0])) * fm[0],
+             fma(xp[1], hps[1] - hpr[sd][1], xc2[1] * (hcs[1] - hcr[sd][1])) * fm[1]);
+    }
+  }
+#undef GEO2
+}
+
+template <int KIND>
+static int launch_k2_lin_kind(const K2Params& p, cudaStream_t st) {
+  const size_t smem = (size_t)K2_NGEO * K2_T * sizeof(double);
+  dim3 grid((unsigned)((p.N + K2_T - 1) / K2_T), (unsigned)((p.B + p.group - 1) / p.group));
+  k2_link_response_lin<KIND><<<grid, K2_THREADS, smem, st>>>(p);
+  LISA_LAUNCH_CHECK("k2_link_response_lin");
+  return LISA_TD_OK;
+}
+static int launch_k2_lin(const K2Params& p, cudaStream_t st) {
+  if (p.orb.kind == 0) return launch_k2_lin_kind<0>(p, st);
+  if (p.orb.kind == 2) return launch_k2_lin_kind<2>(p, st);
+  return launch_k2_lin_kind<1>(p, st);
+}
+
 // A12: y_l[n] = p(n - L_l(t_n)/dt) - p[n].  Small helper kernel, reads p from global memory.
 struct LaserParams {
   long long N;
@@ -348,6 +500,10 @@ int run_link_response(int B, long long N, double t0, double dt, int order, long 
   // |K - Kc| <= |Dl| + drift of Dc over the tile + 1.5; the pair window adds half + 1
   p.halo = (int)ceil((orb.max_off_over_c + orb.max_L) / dt + orb.max_dc_rate * K2_T + 1.5) + p.half + 2;
   make_lags(order, &p.ls);
+  if (!g_force_generic && p.half == 1 && !up2) {  // the paper's linear interpolation: its own kernel
+    p.group = B < K2L_G ? B : K2L_G;
+    return launch_k2_lin(p, st);
+  }
   if (!g_force_generic) {
     switch (p.half) {
       case 1: return launch_k2<1>(p, st);

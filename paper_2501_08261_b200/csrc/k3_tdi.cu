@@ -361,13 +361,15 @@ struct K3Geom {
   // staging area shares its space with y buffer 1, which is first filled after phase 1
   static constexpr int UNION_PRIV = YBUF + (YBUF > CBUF ? YBUF : CBUF);
   static constexpr int UNION_ALIAS = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
-  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= (K3_TS == 16 ? 112 : 227) * 1024;
+  // linear interpolation (H = 1): the stencils are short, two blocks share an SM
+  static constexpr int BLOCKS_PER_SM = (K3_TS == 16 || H == 1) ? 2 : 1;
+  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= (BLOCKS_PER_SM == 2 ? 112 : 227) * 1024;
   static constexpr int UNION = PRIVATE0 ? UNION_PRIV : UNION_ALIAS;
   static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
 };
 
 template <int H, int WIN>
-__global__ void __launch_bounds__(K3_THREADS, K3_TS == 16 ? 2 : 1)
+__global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
     k3_tdi_mma(const K3Params p, const __grid_constant__ CUtensorMap tmap, const int use_tma) {
   using G = K3Geom<H, WIN>;
   constexpr int KCAP = G::KCAP, LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, CS = G::CS, PAD = G::PAD;

@@ -108,6 +108,16 @@ def test_config3_full_size_sampled(lib, orc, orc_d):
     _check_windows(orc, orc_d, inp, tdi, B, N, walkers=(21,), width=2048)
 
 
+def test_order1_full_size_sampled(lib, orc, orc_d):
+    """the paper's linear interpolation (order 1) at B = 64, N = 2^20: the
+    k2_link_response_lin / k3_tdi_mma<1,*> launch configuration the bench times under next.order1"""
+    B, N = 64, 1 << 20
+    inp = synth.make_inputs(3, device="cuda", B=B, N=N)
+    inp["order"] = 1
+    _, _, _, tdi = _gpu_chain_full(lib, inp, B, N)
+    _check_windows(orc, orc_d, inp, tdi, B, N, walkers=(0, 40, 63), width=2048)
+
+
 def test_config4_full_size_loglike(lib, orc_d):
     """configs[3] likelihood at N = 2^20 for two walkers of a full batch-64 launch.  The oracle
     builds its OWN zero-noise injection (walker 0) and its own weights; its fp64 build is used
