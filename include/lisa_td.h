@@ -233,8 +233,9 @@ LISA_TD_API int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, i
 LISA_TD_API int lisa_td_probe_dfma(long long iters, int blocks, int threads, double* sink, float* ms_host,
                        void* stream);
 
-/* Testing switch: non-zero routes S2/S3 through the generic (runtime-order, unmerged) kernels
- * even where a specialised instantiation exists, so the tests can cover both. */
+/* Testing switch: 1 routes S1/S2/S3 through the generic (any mode list, runtime-order, unmerged)
+ * kernels even where a specialised instantiation exists, so the tests can cover both; 2 keeps the
+ * specialised kernels but routes the five-mode S1 through its non-TMA variant; 0 = normal. */
 LISA_TD_API void lisa_td_debug_force_generic(int on);
 
 #ifdef __cplusplus

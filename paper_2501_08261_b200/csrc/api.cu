@@ -239,6 +239,7 @@ int run_loglike(Plan*, int, long long, const double*, const double*, const doubl
 int run_fisher(Plan*, int, long long, const double*, const double*, const double*, long long, long long,
                double*, cudaStream_t);
 extern int g_force_generic;
+extern int g_k1_no_tma;
 
 // ------------------------------------------------------------------ validation helpers
 static int check_common(const char* fn, int B, long long N, double dt, int order) {
@@ -347,7 +348,10 @@ int lisa_td_orbit_table_destroy(lisa_td_orbit_table* t) {
   return LISA_TD_OK;
 }
 int lisa_td_version(void) { return 100; }
-void lisa_td_debug_force_generic(int on) { g_force_generic = on; }
+void lisa_td_debug_force_generic(int on) {
+  g_force_generic = on == 1;
+  g_k1_no_tma = on == 2;
+}
 
 int lisa_td_modes_to_pol(int B, long long N, int n_modes, const int* l_host, const int* m_host,
                          const double* amp, const double* phase, const double* alpha,

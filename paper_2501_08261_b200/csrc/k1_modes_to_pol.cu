@@ -198,6 +198,35 @@ __device__ __forceinline__ K1Pre k1_pre(const quat& q) {
   return r;
 }
 
+// One sample of the five-mode sum: amplitudes / phases of (2,2),(2,1),(3,3),(4,4),(5,5), the
+// monomials of the sample's quaternion, the mode constants, e^{2 i psi}.
+__device__ __forceinline__ void k1_std5_sample(const double (&am)[5], const double (&ph)[5], const K1Pre& pre,
+                                               const double (&cc)[5], double rot_c, double rot_s, double& hp,
+                                               double& hx) {
+  // h_k = a (cos phi - i sin phi), scaled by its constant
+  cplx h[5];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double s, c;
+    const double a = am[k] * cc[k];
+    sincos_d(ph[k], s, c);
+    h[k] = {a * c, -a * s};
+  }
+  // G = h22 + z (h33 + z (h44 + z h55))
+  cplx g = cmul(pre.z, h[4]);
+  g = {g.re + h[3].re, g.im + h[3].im};
+  g = cmul(pre.z, g);
+  g = {g.re + h[2].re, g.im + h[2].im};
+  g = cmul(pre.z, g);
+  g = {g.re + h[0].re, g.im + h[0].im};
+  cplx t1 = cmul(pre.Fa, g), t2 = cmul(pre.Fb, cconj(g));
+  cplx u1 = cmul(pre.qa2, h[1]), u2 = cmul(pre.qb2, cconj(h[1]));
+  cplx u = cmul(pre.qab, {u1.re + u2.re, u1.im + u2.im});
+  const double Hre = (t1.re + t2.re) + u.re, Him = (t1.im + t2.im) + u.im;
+  hp = fma(Hre, rot_c, -Him * rot_s);
+  hx = -fma(Hre, rot_s, Him * rot_c);
+}
+
 // V samples per thread (V = 2: adjacent samples, 16-byte loads and stores; needs even N).  All 13
 // input values of the thread are loaded BEFORE any arithmetic so that each thread has 13 x 8 V
 // bytes in flight (the first version interleaved loads with the sincos evaluations and sat on
@@ -257,28 +286,9 @@ __global__ void __launch_bounds__(K1_THREADS, 3) k1_modes_to_pol_std5(const K1Fa
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     if (p.twisted) pre = k1_pre(quat_mul(quat_from_euler(al[v], be[v], ga[v]), qc));
-    // h_k = a (cos phi - i sin phi), scaled by its constant
-    cplx h[5];
-#pragma unroll
-    for (int k = 0; k < 5; ++k) {
-      double s, c;
-      const double a = am[k][v] * cc[k];
-      sincos_d(ph[k][v], s, c);
-      h[k] = {a * c, -a * s};
-    }
-    // G = h22 + z (h33 + z (h44 + z h55))
-    cplx g = cmul(pre.z, h[4]);
-    g = {g.re + h[3].re, g.im + h[3].im};
-    g = cmul(pre.z, g);
-    g = {g.re + h[2].re, g.im + h[2].im};
-    g = cmul(pre.z, g);
-    g = {g.re + h[0].re, g.im + h[0].im};
-    cplx t1 = cmul(pre.Fa, g), t2 = cmul(pre.Fb, cconj(g));
-    cplx u1 = cmul(pre.qa2, h[1]), u2 = cmul(pre.qb2, cconj(h[1]));
-    cplx u = cmul(pre.qab, {u1.re + u2.re, u1.im + u2.im});
-    const double Hre = (t1.re + t2.re) + u.re, Him = (t1.im + t2.im) + u.im;
-    hp[v] = fma(Hre, rot[0], -Him * rot[1]);
-    hx[v] = -fma(Hre, rot[1], Him * rot[0]);
+    const double amv[5] = {am[0][v], am[1][v], am[2][v], am[3][v], am[4][v]};
+    const double phv[5] = {ph[0][v], ph[1][v], ph[2][v], ph[3][v], ph[4][v]};
+    k1_std5_sample(amv, phv, pre, cc, rot[0], rot[1], hp[v], hx[v]);
   }
   if constexpr (V == 2) {
     *reinterpret_cast<double2*>(p.hplus + bN + n) = make_double2(hp[0], hp[1]);
@@ -286,6 +296,139 @@ __global__ void __launch_bounds__(K1_THREADS, 3) k1_modes_to_pol_std5(const K1Fa
   } else {
     p.hplus[bN + n] = hp[0];
     p.hcross[bN + n] = hx[0];
+  }
+}
+
+// ---------------------------------------------------------------- TMA-pipelined five-mode kernel
+// Persistent blocks (two per SM) walk over (walker, tile of K1T_TILE samples) items.  The 13 input
+// rows of an item arrive in shared memory by 1-D bulk copies (cp.async.bulk, completion counted in
+// bytes on an mbarrier), double buffered: the copies of item i+1 are in flight while item i is
+// evaluated, so the ~330 fp64 operations per sample (8 sincos) and the 104 bytes per sample
+// overlap instead of alternating (the load-everything-first kernel above sits at 64 % of the HBM
+// bandwidth AND 63 % of the fp64 pipe).  Needs even N (16-byte copy sizes and row offsets).
+constexpr int K1T_THREADS = 256;          // measured: 256 x 2 blocks 1.81 ms, 128 x 4 1.83, 64 x 8 and 32 x 16 2.02 (small copies)
+constexpr int K1T_BLOCKS_PER_SM = 2;
+constexpr int K1T_TILE = 2 * K1T_THREADS;  // samples per item: two adjacent samples per thread
+constexpr int K1T_ROWS = 13;              // amp x5, phase x5, alpha, beta, gamma
+constexpr size_t K1T_SMEM = (size_t)2 * K1T_ROWS * K1T_TILE * sizeof(double);
+
+__device__ __forceinline__ unsigned k1_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void k1_bulk_load(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(k1_smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(k1_smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void k1_mbar_wait(uint64_t* b, unsigned parity) {
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(k1_smem_u32(b)), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+
+__global__ void __launch_bounds__(K1T_THREADS, K1T_BLOCKS_PER_SM) k1_modes_to_pol_std5_tma(const K1FastParams p, const int tiles_per_row,
+                                                                        const long long n_items) {
+  extern __shared__ __align__(128) double k1_stage[];  // [2][K1T_ROWS][K1T_TILE]
+  __shared__ __align__(8) uint64_t bar[2];
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(k1_smem_u32(&bar[0])) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(k1_smem_u32(&bar[1])) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  // one thread issues the copies of an item: present modes and, if twisted, the three angles
+  auto issue = [&](long long item, int stage) {
+    const int b = (int)(item / tiles_per_row);
+    const long long n0 = (item % tiles_per_row) * K1T_TILE;
+    const unsigned bytes = (unsigned)(min((long long)K1T_TILE, p.N - n0) * sizeof(double));
+    int rows = p.twisted ? 3 : 0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) rows += p.idx[k] >= 0 ? 2 : 0;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(k1_smem_u32(&bar[stage])), "r"(bytes * rows)
+                 : "memory");
+    double* dst = k1_stage + (size_t)stage * K1T_ROWS * K1T_TILE;
+    const size_t bN = (size_t)b * p.N;
+#pragma unroll
+    for (int k = 0; k < 5; ++k)
+      if (p.idx[k] >= 0) {
+        const size_t off = (bN * p.n_modes + (size_t)p.idx[k] * p.N) + n0;
+        k1_bulk_load(dst + k * K1T_TILE, p.amp + off, bytes, &bar[stage]);
+        k1_bulk_load(dst + (5 + k) * K1T_TILE, p.phase + off, bytes, &bar[stage]);
+      }
+    if (p.twisted) {
+      k1_bulk_load(dst + 10 * K1T_TILE, p.alpha + bN + n0, bytes, &bar[stage]);
+      k1_bulk_load(dst + 11 * K1T_TILE, p.beta + bN + n0, bytes, &bar[stage]);
+      k1_bulk_load(dst + 12 * K1T_TILE, p.gamma + bN + n0, bytes, &bar[stage]);
+    }
+  };
+  if (threadIdx.x == 0 && blockIdx.x < n_items) issue(blockIdx.x, 0);
+
+  const double cc[5] = {p.c22, p.c21, p.c33, p.c44, p.c55};
+  quat qc = {{1.0, 0.0}, {0.0, 0.0}};
+  double rot_c = 1.0, rot_s = 0.0;
+  K1Pre pre = k1_pre(qc);
+  int b_have = -1;
+  int it = 0;
+  for (long long item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+    const int stage = it & 1;
+    // every thread is past its reads of the other stage (barrier at the end of the last round)
+    if (threadIdx.x == 0 && item + gridDim.x < n_items) issue(item + gridDim.x, stage ^ 1);
+    const int b = (int)(item / tiles_per_row);
+    const long long n = (item % tiles_per_row) * K1T_TILE + 2 * threadIdx.x;
+    if (b != b_have) {  // per-walker constants (uniform branch; a walker spans many items)
+      qc = quat_from_euler(p.phi[b], p.iota[b], 0.0);  // footnote 1
+      if (p.have_e0) qc = quat_mul(quat_from_euler(p.euler0[3 * b], p.euler0[3 * b + 1], p.euler0[3 * b + 2]), qc);
+      sincos_d(2.0 * p.psi[b], rot_s, rot_c);
+      pre = k1_pre(qc);
+      b_have = b;
+    }
+    k1_mbar_wait(&bar[stage], (unsigned)((it >> 1) & 1));
+    if (n < p.N) {
+      const double* src = k1_stage + (size_t)stage * K1T_ROWS * K1T_TILE + 2 * threadIdx.x;
+      double2 am2[5], ph2[5];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        am2[k] = ph2[k] = make_double2(0.0, 0.0);
+        if (p.idx[k] >= 0) {
+          am2[k] = *reinterpret_cast<const double2*>(src + k * K1T_TILE);
+          ph2[k] = *reinterpret_cast<const double2*>(src + (5 + k) * K1T_TILE);
+        }
+      }
+      double hp[2], hx[2];
+      if (p.twisted) {
+        const double2 al = *reinterpret_cast<const double2*>(src + 10 * K1T_TILE);
+        const double2 be = *reinterpret_cast<const double2*>(src + 11 * K1T_TILE);
+        const double2 ga = *reinterpret_cast<const double2*>(src + 12 * K1T_TILE);
+        {
+          const double amv[5] = {am2[0].x, am2[1].x, am2[2].x, am2[3].x, am2[4].x};
+          const double phv[5] = {ph2[0].x, ph2[1].x, ph2[2].x, ph2[3].x, ph2[4].x};
+          k1_std5_sample(amv, phv, k1_pre(quat_mul(quat_from_euler(al.x, be.x, ga.x), qc)), cc, rot_c, rot_s, hp[0], hx[0]);
+        }
+        {
+          const double amv[5] = {am2[0].y, am2[1].y, am2[2].y, am2[3].y, am2[4].y};
+          const double phv[5] = {ph2[0].y, ph2[1].y, ph2[2].y, ph2[3].y, ph2[4].y};
+          k1_std5_sample(amv, phv, k1_pre(quat_mul(quat_from_euler(al.y, be.y, ga.y), qc)), cc, rot_c, rot_s, hp[1], hx[1]);
+        }
+      } else {
+        const double amx[5] = {am2[0].x, am2[1].x, am2[2].x, am2[3].x, am2[4].x};
+        const double phx[5] = {ph2[0].x, ph2[1].x, ph2[2].x, ph2[3].x, ph2[4].x};
+        k1_std5_sample(amx, phx, pre, cc, rot_c, rot_s, hp[0], hx[0]);
+        const double amy[5] = {am2[0].y, am2[1].y, am2[2].y, am2[3].y, am2[4].y};
+        const double phy[5] = {ph2[0].y, ph2[1].y, ph2[2].y, ph2[3].y, ph2[4].y};
+        k1_std5_sample(amy, phy, pre, cc, rot_c, rot_s, hp[1], hx[1]);
+      }
+      const size_t o = (size_t)b * p.N + n;
+      *reinterpret_cast<double2*>(p.hplus + o) = make_double2(hp[0], hp[1]);
+      *reinterpret_cast<double2*>(p.hcross + o) = make_double2(hx[0], hx[1]);
+    }
+    __syncthreads();  // this stage may be refilled from the next round on
   }
 }
 
@@ -302,6 +445,7 @@ static long double binom_ld(int n, int k) {
 }
 
 extern int g_force_generic;
+int g_k1_no_tma = 0;  // debug switch (lisa_td_debug_force_generic(2)): the load-everything-first five-mode kernel
 
 int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m, const double* amp,
                      const double* phase, const double* alpha, const double* beta,
@@ -331,7 +475,16 @@ int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m
       f.B = B; f.N = N; f.n_modes = n_modes; f.twisted = alpha != nullptr; f.have_e0 = euler0 != nullptr;
       f.amp = amp; f.phase = phase; f.alpha = alpha; f.beta = beta; f.gamma = gamma;
       f.iota = iota; f.phi = phi; f.psi = psi; f.euler0 = euler0; f.hplus = hplus; f.hcross = hcross;
-      if ((N & 1) == 0) {
+      if ((N & 1) == 0 && !g_k1_no_tma) {
+        const int tiles_per_row = (int)((N + K1T_TILE - 1) / K1T_TILE);
+        const long long n_items = (long long)tiles_per_row * B;
+        int dev = 0, sms = 148;
+        LISA_CUDA(cudaGetDevice(&dev));
+        LISA_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        const long long blocks = n_items < (long long)K1T_BLOCKS_PER_SM * sms ? n_items : (long long)K1T_BLOCKS_PER_SM * sms;
+        LISA_CUDA(cudaFuncSetAttribute(k1_modes_to_pol_std5_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K1T_SMEM));
+        k1_modes_to_pol_std5_tma<<<(unsigned)blocks, K1T_THREADS, K1T_SMEM, st>>>(f, tiles_per_row, n_items);
+      } else if ((N & 1) == 0) {
         dim3 grid((unsigned)((N / 2 + K1_THREADS - 1) / K1_THREADS), (unsigned)B);
         k1_modes_to_pol_std5<2><<<grid, K1_THREADS, 0, st>>>(f);
       } else {

@@ -183,7 +183,7 @@ def version() -> int:
 
 
 def debug_force_generic(on: bool):
-    load().lisa_td_debug_force_generic(int(bool(on)))
+    load().lisa_td_debug_force_generic(int(on))
 
 
 def modes_to_pol(B, N, l, m, amp, phase, alpha, beta, gamma, iota, phi, psi, euler0, hplus, hcross):

@@ -79,13 +79,14 @@ def _s1_inputs(rng, modes, B, N, big_phase=True):
 @pytest.mark.parametrize("modes", [[(2, 2)], MODES5, MODES_GEN])
 @pytest.mark.parametrize("twisted", [False, True])
 @pytest.mark.parametrize("with_e0", [False, True])
-@pytest.mark.parametrize("force_generic", [False, True])
+@pytest.mark.parametrize("force_generic", [0, 1, 2])
 def test_s1_parity(lib, orc, modes, twisted, with_e0, force_generic):
-    """force_generic=False takes the five-mode fast kernel for the first two mode lists."""
+    """force_generic=0 takes the five-mode TMA-pipelined kernel for the first two mode lists (N even),
+    2 its load-everything-first variant, 1 the generic kernel."""
     if force_generic and len(modes) > 5:
         pytest.skip("already the generic kernel")
     rng = np.random.default_rng(11 + len(modes) + 2 * twisted + with_e0)
-    B, N = 3, 2500  # several blocks and a ragged tail
+    B, N = 3, 2500  # several blocks / items and a ragged tail
     l, m = zip(*modes)
     amp, phase, iota, phi, psi = _s1_inputs(rng, modes, B, N)
     ang = [rng.uniform(-400, 400, (B, N)), rng.uniform(0, math.pi, (B, N)), rng.uniform(-400, 400, (B, N))] if twisted else [None] * 3
@@ -95,12 +96,32 @@ def test_s1_parity(lib, orc, modes, twisted, with_e0, force_generic):
     try:
         got = gpu_s1(lib, l, m, amp, phase, iota, phi, psi, *ang, euler0=e0)
     finally:
-        lib.debug_force_generic(False)
+        lib.debug_force_generic(0)
     scale = np.sum(amp, axis=1)
     for g, r in zip(got, ref):
         # up to l+2 = 10 chained complex products per row and 2 n_modes rows: a few 1e-16 each
         assert np.max(np.abs(g - r) / scale) < 2e-14
         assert rel_l2(g, r) < 5e-15
+
+
+@pytest.mark.parametrize("B,N", [(5, 1 << 16), (2, 1026), (3, 2501)])
+def test_s1_five_mode_kernels_agree_bitwise(lib, B, N):
+    """the TMA-pipelined persistent kernel (every block walks many (walker, tile) items when there are
+    more than 296 of them; ragged last tile) against the load-everything-first kernel: same
+    arithmetic, same bits; odd N takes the one-sample-per-thread variant in both modes"""
+    rng = np.random.default_rng(N)
+    l, m = zip(*MODES5)
+    amp, phase, iota, phi, psi = _s1_inputs(rng, MODES5, B, N)
+    ang = [rng.uniform(-400, 400, (B, N)), rng.uniform(0, math.pi, (B, N)), rng.uniform(-400, 400, (B, N))]
+    outs = []
+    for mode in (0, 2):
+        lib.debug_force_generic(mode)
+        try:
+            outs.append(gpu_s1(lib, l, m, amp, phase, iota, phi, psi, *ang, euler0=None))
+        finally:
+            lib.debug_force_generic(0)
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert np.all(np.isfinite(outs[0][0])) and np.abs(outs[0][0]).max() > 0.0
 
 
 def test_s1_beta_pi(lib, orc):
