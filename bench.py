@@ -257,6 +257,14 @@ def run_ours(args):
     ms = lib.probe_dfma(iters, 148 * 8, 256, sink)
     dfma_peak_tflops = 2 * 8 * iters * 148 * 8 * 256 / (ms * 1e-3) / 1e12
 
+    # do the DFMA pipe (K1, K2) and the fp64 tensor path (K3) run side by side?  8 + 8 warps per SM
+    pipes = {}
+    for name, (nf_w, nm_w) in (("dfma_only", (8, 0)), ("dmma_only", (0, 8)), ("both", (8, 8))):
+        lib.probe_fp64_pipes(2000, 148, nf_w, nm_w, sink)
+        pms = lib.probe_fp64_pipes(100000, 148, nf_w, nm_w, sink)
+        pipes[name] = {"ms": pms, "tflops": 2 * 100000 * 148 * (256 * nf_w + 1024 * nm_w) / (pms * 1e-3) / 1e12}
+    pipes["reading"] = "times add: one fp64 resource" if pipes["both"]["ms"] > 0.9 * (pipes["dfma_only"]["ms"] + pipes["dmma_only"]["ms"]) else "overlap"
+
     stages = [("S1_modes_to_pol", s1), ("S2_link_response", s2), ("S3_tdi2", s3), ("S45_fft_loglike", s45)]
     for _ in range(max(args.warmup, 3)):
         for _, fn in stages:
@@ -468,7 +476,7 @@ def run_ours(args):
         "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
             "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
-        "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops,
+        "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops, "fp64_pipes": pipes,
         "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info,
                  "order1": order1_info},
     }

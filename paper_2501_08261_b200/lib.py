@@ -24,7 +24,7 @@ EXPORTS = [
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
     "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
-    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_probe_dfma",
+    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_probe_dfma", "lisa_td_probe_fp64_pipes",
     "lisa_td_debug_force_generic",
 ]
 
@@ -132,6 +132,7 @@ def load() -> C.CDLL:
                                         + [dbl, dbl, i32, i64, i32, i64, i64, C.POINTER(Orbit), vp, vp,
                                            i64, i64, vp, vp, vp])
     L.lisa_td_probe_dfma.argtypes = [i64, i32, i32, vp, C.POINTER(C.c_float), vp]
+    L.lisa_td_probe_fp64_pipes.argtypes = [i64, i32, i32, i32, vp, C.POINTER(C.c_float), vp]
     L.lisa_td_debug_force_generic.argtypes = [i32]
     L.lisa_td_debug_force_generic.restype = None
     _lib = L
@@ -308,4 +309,10 @@ def pipeline_host(pipe: Pipeline, B, N, l, m, amp, phase, alpha, beta, gamma, io
 def probe_dfma(iters, blocks, threads, sink) -> float:
     ms = C.c_float()
     _check(load().lisa_td_probe_dfma(iters, blocks, threads, _dev(sink), C.byref(ms), _stream()))
+    return ms.value
+
+
+def probe_fp64_pipes(iters, blocks, dfma_warps, dmma_warps, sink) -> float:
+    ms = C.c_float()
+    _check(load().lisa_td_probe_fp64_pipes(iters, blocks, dfma_warps, dmma_warps, _dev(sink), C.byref(ms), _stream()))
     return ms.value
