@@ -186,13 +186,11 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 
   for (int w = 0; w < nw; ++w) {
     const int buf = w & 1;
-    if (w + 1 < nw) {
-      prefetch(w + 1, buf ^ 1);
-      asm volatile("cp.async.wait_group 1;\n" ::);
-    } else {
-      asm volatile("cp.async.wait_group 0;\n" ::);
-    }
-    __syncthreads();  // tile of walker w (and, first time round, geo[]) visible to everyone
+    asm volatile("cp.async.wait_group 0;\n" ::);
+    // ONE barrier per walker: the tile of walker w (and, first time round, geo[]) is visible to everyone,
+    // and everyone is done reading the other buffer (walker w-1), so it can be refilled right away
+    __syncthreads();
+    if (w + 1 < nw) prefetch(w + 1, buf ^ 1);
     double* yb = p.y + (size_t)(w0 + w) * 6 * p.N + na;
     auto store2 = [&](int l, double v0, double v1) {
       double* dst = yb + (size_t)l * p.N;
@@ -250,7 +248,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 #pragma unroll 1
       for (int k = 0; k < 3; ++k) {  // slot 0 holds spacecraft k
         read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd[0][0], kd[0][1], p, hpr[0], hcr[0]);
-        ROT3(kd); ROT3(ud); ROT3(vd); ROT3(hpr); ROT3(hcr);
+        ROT3(kd); ROT3(hpr); ROT3(hcr);  // ud, vd are not read here and three rotations are the identity
       }
       // three arms; links a and -a share x+, xx and have opposite n.  Arm a joins spacecraft
       // link_s(a) = a+2 and link_r(a) = a+1 (mod 3): after a rotations they sit in slots 2, 1.
@@ -285,7 +283,6 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
 #pragma unroll
       for (int l = 0; l < 6; ++l) store2(l, 0.0, 0.0);
     }
-    __syncthreads();  // everyone is done with buffer `buf` before walker w+2 is prefetched into it
   }
 #undef GEO2
 }
