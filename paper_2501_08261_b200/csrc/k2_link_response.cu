@@ -20,8 +20,9 @@ namespace lisa {
 
 constexpr int K2_T = 256;        // output samples per block
 constexpr int K2_THREADS = 128;  // two adjacent samples per thread
-constexpr int K2_G = 16;         // walkers per block (upper bound)
+constexpr int K2_G = 16;         // walkers per block (upper bound; 32 measured the same)
 constexpr int K2_NGEO = 21;      // geometry fields per sample
+constexpr bool K2_RMAJOR = true;  // receiver-major sweep order (see the kernel)
 
 struct K2Params {
   int B;
@@ -222,6 +223,56 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
           Dc[1] = fma(kz, g2.y, Dc[1]);
         }
       }
+      if constexpr (K2_RMAJOR) {
+        // Receiver-major order: iteration k handles spacecraft k as RECEIVER -- its reception-time read
+        // and the two links it receives: link +(k+2) from spacecraft k+1 and link -(k+1) from spacecraft
+        // k+2 (indices mod 3).  The offsets of the three spacecraft are re-read from geo[] by runtime
+        // field index each time, so no per-slot state lives across iterations: no slot rotation, and
+        // ~50 fewer live registers during the sweeps (the price: arm projections are formed per link
+        // instead of per arm, +75 fp64 operations per walker-sample).
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+          const int k1 = k == 2 ? 0 : k + 1, k2 = k == 0 ? 2 : k - 1;
+          double kd0[2], DsA[2], DsB[2], xpA[2], xcA[2], fA[2], xpB[2], xcB[2], fB[2];
+          {
+            const double2 rx = GEO2(2 + 3 * k), ry = GEO2(3 + 3 * k), rz = GEO2(4 + 3 * k);
+            const double2 ax = GEO2(2 + 3 * k1), ay = GEO2(3 + 3 * k1), az = GEO2(4 + 3 * k1);
+            const double2 bx = GEO2(2 + 3 * k2), by = GEO2(3 + 3 * k2), bz = GEO2(4 + 3 * k2);
+            const double2 LA = GEO2(11 + k2), ilA = GEO2(17 + k2);  // link +(k+2): k1 -> k
+            const double2 LB = GEO2(14 + k1), ilB = GEO2(17 + k1);  // link -(k+1): k2 -> k
+            const double rxs[2] = {rx.x, rx.y}, rys[2] = {ry.x, ry.y}, rzs[2] = {rz.x, rz.y};
+            const double eAx[2] = {rx.x - ax.x, rx.y - ax.y}, eAy[2] = {ry.x - ay.x, ry.y - ay.y}, eAz[2] = {rz.x - az.x, rz.y - az.y};
+            const double eBx[2] = {rx.x - bx.x, rx.y - bx.y}, eBy[2] = {ry.x - by.x, ry.y - by.y}, eBz[2] = {rz.x - bz.x, rz.y - bz.y};
+            const double LAs[2] = {LA.x, LA.y}, LBs[2] = {LB.x, LB.y}, ilAs[2] = {ilA.x, ilA.y}, ilBs[2] = {ilB.x, ilB.y};
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+              kd0[c] = fma(kx, rxs[c], fma(ky, rys[c], kz * rzs[c]));
+              const double keA = fma(kx, eAx[c], fma(ky, eAy[c], kz * eAz[c]));  // k.(r_k - r_k1)
+              const double keB = fma(kx, eBx[c], fma(ky, eBy[c], kz * eBz[c]));
+              DsA[c] = LAs[c] + (kd0[c] - keA);  // L + k.r_sender
+              DsB[c] = LBs[c] + (kd0[c] - keB);
+              const double unA = fma(ux, eAx[c], uy * eAy[c]) * ilAs[c], vnA = fma(vx, eAx[c], fma(vy, eAy[c], vz * eAz[c])) * ilAs[c];
+              const double unB = fma(ux, eBx[c], uy * eBy[c]) * ilBs[c], vnB = fma(vx, eBx[c], fma(vy, eBy[c], vz * eBz[c])) * ilBs[c];
+              xpA[c] = fma(unA, unA, -vnA * vnA);
+              xcA[c] = 2.0 * unA * vnA;
+              xpB[c] = fma(unB, unB, -vnB * vnB);
+              xcB[c] = 2.0 * unB * vnB;
+              const double omA = 1.0 - keA * ilAs[c], omB = 1.0 - keB * ilBs[c];  // 1 - k.n of each link
+              const double inv = 0.5 / (omA * omB);
+              fA[c] = omB * inv;
+              fB[c] = omA * inv;
+            }
+          }
+          double hpr[2], hcr[2], hps[2], hcs[2];
+          read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd0[0], kd0[1], p, hpr, hcr);
+          read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, DsA[0], DsA[1], p, hps, hcs);
+          store2(k2, fma(xpA[0], hps[0] - hpr[0], xcA[0] * (hcs[0] - hcr[0])) * fA[0],
+                 fma(xpA[1], hps[1] - hpr[1], xcA[1] * (hcs[1] - hcr[1])) * fA[1]);
+          read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, DsB[0], DsB[1], p, hps, hcs);
+          store2(k1 + 3, fma(xpB[0], hps[0] - hpr[0], xcB[0] * (hcs[0] - hcr[0])) * fB[0],
+                 fma(xpB[1], hps[1] - hpr[1], xcB[1] * (hcs[1] - hcr[1])) * fB[1]);
+        }
+      } else {
       // per spacecraft slot: k.offset, u.offset, v.offset (samples) and the reception-time
       // reads h(t - k.r_r/c).  The loops below are NOT unrolled (the unrolled body overflowed
       // the instruction cache); instead the three slots are rotated after every pass, so the
@@ -279,6 +330,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
         ROT3(kd); ROT3(ud); ROT3(vd); ROT3(hpr); ROT3(hcr);
       }
 #undef ROT3
+      }
     } else {
 #pragma unroll
       for (int l = 0; l < 6; ++l) store2(l, 0.0, 0.0);
