@@ -18,7 +18,10 @@
  *    lisa_td_plan.  Inputs are never modified.
  *  - Every call only ENQUEUES work on `stream` (a cudaStream_t passed as void*; NULL = the
  *    legacy default stream) and returns without synchronising, except lisa_td_plan_create /
- *    lisa_td_plan_destroy, lisa_td_pipeline_host and lisa_td_probe_dfma, which synchronise.
+ *    lisa_td_plan_destroy, lisa_td_orbit_table_create, lisa_td_pipeline_host and the lisa_td_probe_*
+ *    calls, which synchronise.  The enqueue-only calls may therefore be captured into a CUDA graph
+ *    and replayed (tests/test_gpu_graph.py; call lisa_td_loglike once with the batch size before
+ *    capturing: the first use of a batch size creates its cuFFT plan).
  *  - Return value: LISA_TD_OK (0) or a negative lisa_td_status.  Argument errors are detected
  *    on the host before any launch.  The library never throws, aborts or falls back to the
  *    CPU.  lisa_td_last_error() returns a thread-local description of the last failure.
