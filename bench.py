@@ -456,6 +456,26 @@ def run_ours(args):
         e2e = {"value": B / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(B * 8),
                "ms_per_step": t_e2e * 1e3, "api": "lisa_td_pipeline_host (chunks of 16 walkers, copy/compute streams)",
                "steps": n_e2e}
+        # the same call with the paper's 10 s sampling of the modes: half the bytes cross PCIe
+        cz = lambda t: torch.cat([t[..., ::2], t[..., -1:]], dim=-1).contiguous().pin_memory()
+        host_c = {k: cz(host[k]) for k in ("amp", "phase", "alpha", "beta", "gamma")}
+        out_c = torch.empty(B, dtype=f64).pin_memory()
+
+        def e2e_up2_step():
+            lib.pipeline_host_up2(pipe, B, N, inp["l"], inp["m"], host_c["amp"], host_c["phase"], host_c["alpha"],
+                                  host_c["beta"], host_c["gamma"], host["iota"], host["phi"], host["psi"], host["lam"],
+                                  host["beta_sky"], t0, dt, ORDER, inp["margin_y"], 20, inp["margin_lo"],
+                                  inp["margin_hi"], inp["orbit"], data_h, w_h, kmin, kmax, out_c)
+        e2e_up2_step()
+        t_start = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_up2_step()
+        t_up2 = (time.perf_counter() - t_start) / n_e2e
+        e2e["up2"] = {"value": B / t_up2, "unit": UNIT, "ms_per_step": t_up2 * 1e3,
+                      "h2d_bytes_per_step": int(sum(host_c[k].numel() for k in host_c) * 8 + (data_h.numel() + w_h.numel()) * 8),
+                      "api": "lisa_td_pipeline_host_up2 (modes on the 10 s grid, PAPER.md:243; a different, coarser input: not the headline)",
+                      "loglike_walker0_rel_diff": abs(float(out_c[0]) - loglike0) / abs(loglike0)}
+        del host_c
         pipe.close()
 
     # ---- the oracle beside it (bounded sample, host cores)

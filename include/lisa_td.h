@@ -229,6 +229,22 @@ LISA_TD_API int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, i
                           const double* weight_host, long long kmin, long long kmax,
                           double* loglike_host, double* dh_host, double* hh_host);
 
+/* The same with the paper's 10 s -> 5 s trick (reading A20): amp/phase_host are
+ * [B][n_modes][N/2+1] and alpha/beta/gamma_host [B][N/2+1], sampled on the grid t0 + i (2 dt); S1 runs
+ * on that grid and S2 interpolates h+, hx linearly to the dt grid (lisa_td_link_response_up2).  Half
+ * the bytes cross PCIe.  Everything else (N, margins, data, weights, outputs) as above. */
+LISA_TD_API int lisa_td_pipeline_host_up2(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                              const int* m_host, const double* amp_host, const double* phase_host,
+                              const double* alpha_host, const double* beta_host,
+                              const double* gamma_host, const double* iota_host,
+                              const double* phi_host, const double* psi_host,
+                              const double* lambda_host, const double* beta_sky_host, double t0,
+                              double dt, int order, long long margin_y, int generation,
+                              long long margin_lo, long long margin_hi,
+                              const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                              const double* weight_host, long long kmin, long long kmax,
+                              double* loglike_host, double* dh_host, double* hh_host);
+
 /* Measurement support: a register-resident chain of `iters` x 8 dependent-free DFMA per thread on
  * `blocks` x `threads`; returns the elapsed milliseconds (CUDA events) in *ms_host and writes one
  * double per thread to sink (device, blocks*threads doubles) so the work is not optimised away.

@@ -616,7 +616,7 @@ int lisa_td_pipeline_create(lisa_td_pipeline** out, int chunk_B, long long N, in
   memset(p, 0, sizeof(*p));
   p->chunk_B = chunk_B; p->N = N; p->nf = N / 2 + 1; p->n_modes = n_modes; p->twisted = twisted;
   const size_t cB = chunk_B;
-  p->in_doubles = cB * (2 * (size_t)n_modes + (twisted ? 3 : 0)) * N + 8 * cB + 16;
+  p->in_doubles = cB * (2 * (size_t)n_modes + (twisted ? 3 : 0)) * N + 8 * cB + 32;
   int rc = LISA_TD_OK;
 #define PIPE_TRY(call) do { if (rc == LISA_TD_OK) rc = check_cuda((call), #call); } while (0)
   PIPE_TRY(cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking));
@@ -643,18 +643,17 @@ int lisa_td_pipeline_create(lisa_td_pipeline** out, int chunk_B, long long N, in
   return LISA_TD_OK;
 }
 
-int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
-                          const int* m_host, const double* amp_host, const double* phase_host,
-                          const double* alpha_host, const double* beta_host,
-                          const double* gamma_host, const double* iota_host,
-                          const double* phi_host, const double* psi_host,
-                          const double* lambda_host, const double* beta_sky_host, double t0,
-                          double dt, int order, long long margin_y, int generation,
-                          long long margin_lo, long long margin_hi,
-                          const lisa_td_orbit* orbit_host, const double* data_spec_host,
-                          const double* weight_host, long long kmin, long long kmax,
-                          double* loglike_host, double* dh_host, double* hh_host) {
-  const char* fn = "lisa_td_pipeline_host";
+static int pipeline_run(const char* fn, int up2, lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                        const int* m_host, const double* amp_host, const double* phase_host,
+                        const double* alpha_host, const double* beta_host,
+                        const double* gamma_host, const double* iota_host,
+                        const double* phi_host, const double* psi_host,
+                        const double* lambda_host, const double* beta_sky_host, double t0,
+                        double dt, int order, long long margin_y, int generation,
+                        long long margin_lo, long long margin_hi,
+                        const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                        const double* weight_host, long long kmin, long long kmax,
+                        double* loglike_host, double* dh_host, double* hh_host) {
   if (!p) return set_error(LISA_TD_EINVAL, "%s: pipeline is NULL", fn);
   int rc = check_common(fn, B, N, dt, order);
   if (rc) return rc;
@@ -675,6 +674,10 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
   if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
 
   const size_t M = n_modes, cB = p->chunk_B;
+  // up2 (reading A20): the mode and angle arrays live on the 2 dt grid, Nin = N/2 + 1 samples
+  // per row; sub-arrays start on even offsets so that every device array stays 16-byte aligned
+  const size_t Nin = up2 ? (size_t)(N / 2 + 1) : (size_t)N;
+  auto even = [](size_t v) { return (v + 1) & ~(size_t)1; };
   LISA_CUDA(cudaMemcpyAsync(p->data_spec, data_spec_host, sizeof(double) * 6 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
   LISA_CUDA(cudaMemcpyAsync(p->weight, weight_host, sizeof(double) * 3 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
   int it = 0;
@@ -683,21 +686,21 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
     const size_t nb = (size_t)((B - b0) < (int)cB ? (B - b0) : (int)cB);
     double* d = p->in[buf];
     double* d_amp = d;
-    double* d_pha = d_amp + cB * M * N;
-    double* d_al = d_pha + cB * M * N;
-    double* d_be = d_al + (tw ? cB * N : 0);
-    double* d_ga = d_be + (tw ? cB * N : 0);
-    double* d_sc = d_ga + (tw ? cB * N : 0);  // 5 x [cB] scalars, each slot padded to 2*... keep 16B aligned
+    double* d_pha = d_amp + even(cB * M * Nin);
+    double* d_al = d_pha + even(cB * M * Nin);
+    double* d_be = d_al + (tw ? even(cB * Nin) : 0);
+    double* d_ga = d_be + (tw ? even(cB * Nin) : 0);
+    double* d_sc = d_ga + (tw ? even(cB * Nin) : 0);  // 5 x [cB] scalars, each slot padded to an even count
     const size_t sc_stride = (cB + 1) & ~(size_t)1;
     // copies of chunk `it` wait until the kernels that last used this buffer are done
     if (it >= 2) LISA_CUDA(cudaStreamWaitEvent(p->s_copy, p->done[buf], 0));
 #define H2D(dst, src, count) LISA_CUDA(cudaMemcpyAsync((dst), (src), sizeof(double) * (count), cudaMemcpyHostToDevice, p->s_copy))
-    H2D(d_amp, amp_host + (size_t)b0 * M * N, nb * M * N);
-    H2D(d_pha, phase_host + (size_t)b0 * M * N, nb * M * N);
+    H2D(d_amp, amp_host + (size_t)b0 * M * Nin, nb * M * Nin);
+    H2D(d_pha, phase_host + (size_t)b0 * M * Nin, nb * M * Nin);
     if (tw) {
-      H2D(d_al, alpha_host + (size_t)b0 * N, nb * N);
-      H2D(d_be, beta_host + (size_t)b0 * N, nb * N);
-      H2D(d_ga, gamma_host + (size_t)b0 * N, nb * N);
+      H2D(d_al, alpha_host + (size_t)b0 * Nin, nb * Nin);
+      H2D(d_be, beta_host + (size_t)b0 * Nin, nb * Nin);
+      H2D(d_ga, gamma_host + (size_t)b0 * Nin, nb * Nin);
     }
     H2D(d_sc + 0 * sc_stride, iota_host + b0, nb);
     H2D(d_sc + 1 * sc_stride, phi_host + b0, nb);
@@ -707,12 +710,12 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
 #undef H2D
     LISA_CUDA(cudaEventRecord(p->copied[buf], p->s_copy));
     LISA_CUDA(cudaStreamWaitEvent(p->s_comp, p->copied[buf], 0));
-    if ((rc = run_modes_to_pol((int)nb, N, n_modes, l_host, m_host, d_amp, d_pha, tw ? d_al : nullptr,
+    if ((rc = run_modes_to_pol((int)nb, (long long)Nin, n_modes, l_host, m_host, d_amp, d_pha, tw ? d_al : nullptr,
                                tw ? d_be : nullptr, tw ? d_ga : nullptr, d_sc, d_sc + sc_stride,
                                d_sc + 2 * sc_stride, nullptr, p->hp, p->hc, p->s_comp)))
       return rc;
     if ((rc = run_link_response((int)nb, N, t0, dt, order, margin_y, p->hp, p->hc, d_sc + 3 * sc_stride,
-                                d_sc + 4 * sc_stride, od, p->y, p->s_comp)))
+                                d_sc + 4 * sc_stride, od, p->y, p->s_comp, up2)))
       return rc;
     if ((rc = run_tdi((int)nb, N, t0, dt, order, generation, 1, margin_lo, margin_hi, p->y, od, p->tdi, p->s_comp)))
       return rc;
@@ -727,6 +730,40 @@ int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, 
   LISA_CUDA(cudaStreamSynchronize(p->s_copy));
   LISA_CUDA(cudaStreamSynchronize(p->s_comp));
   return LISA_TD_OK;
+}
+
+int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                          const int* m_host, const double* amp_host, const double* phase_host,
+                          const double* alpha_host, const double* beta_host,
+                          const double* gamma_host, const double* iota_host,
+                          const double* phi_host, const double* psi_host,
+                          const double* lambda_host, const double* beta_sky_host, double t0,
+                          double dt, int order, long long margin_y, int generation,
+                          long long margin_lo, long long margin_hi,
+                          const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                          const double* weight_host, long long kmin, long long kmax,
+                          double* loglike_host, double* dh_host, double* hh_host) {
+  return pipeline_run("lisa_td_pipeline_host", 0, p, B, N, n_modes, l_host, m_host, amp_host, phase_host, alpha_host,
+                      beta_host, gamma_host, iota_host, phi_host, psi_host, lambda_host, beta_sky_host, t0, dt, order,
+                      margin_y, generation, margin_lo, margin_hi, orbit_host, data_spec_host, weight_host, kmin, kmax,
+                      loglike_host, dh_host, hh_host);
+}
+
+int lisa_td_pipeline_host_up2(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
+                              const int* m_host, const double* amp_host, const double* phase_host,
+                              const double* alpha_host, const double* beta_host,
+                              const double* gamma_host, const double* iota_host,
+                              const double* phi_host, const double* psi_host,
+                              const double* lambda_host, const double* beta_sky_host, double t0,
+                              double dt, int order, long long margin_y, int generation,
+                              long long margin_lo, long long margin_hi,
+                              const lisa_td_orbit* orbit_host, const double* data_spec_host,
+                              const double* weight_host, long long kmin, long long kmax,
+                              double* loglike_host, double* dh_host, double* hh_host) {
+  return pipeline_run("lisa_td_pipeline_host_up2", 1, p, B, N, n_modes, l_host, m_host, amp_host, phase_host, alpha_host,
+                      beta_host, gamma_host, iota_host, phi_host, psi_host, lambda_host, beta_sky_host, t0, dt, order,
+                      margin_y, generation, margin_lo, margin_hi, orbit_host, data_spec_host, weight_host, kmin, kmax,
+                      loglike_host, dh_host, hh_host);
 }
 
 // ---------------------------------------------------------------------- DFMA probe

@@ -24,7 +24,7 @@ EXPORTS = [
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
     "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
-    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_probe_dfma", "lisa_td_probe_fp64_pipes",
+    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_pipeline_host_up2", "lisa_td_probe_dfma", "lisa_td_probe_fp64_pipes",
     "lisa_td_debug_force_generic",
 ]
 
@@ -131,6 +131,7 @@ def load() -> C.CDLL:
     L.lisa_td_pipeline_host.argtypes = ([vp, i32, i64, i32, C.POINTER(i32), C.POINTER(i32)] + [vp] * 10
                                         + [dbl, dbl, i32, i64, i32, i64, i64, C.POINTER(Orbit), vp, vp,
                                            i64, i64, vp, vp, vp])
+    L.lisa_td_pipeline_host_up2.argtypes = L.lisa_td_pipeline_host.argtypes
     L.lisa_td_probe_dfma.argtypes = [i64, i32, i32, vp, C.POINTER(C.c_float), vp]
     L.lisa_td_probe_fp64_pipes.argtypes = [i64, i32, i32, i32, vp, C.POINTER(C.c_float), vp]
     L.lisa_td_debug_force_generic.argtypes = [i32]
@@ -302,6 +303,18 @@ def pipeline_host(pipe: Pipeline, B, N, l, m, amp, phase, alpha, beta, gamma, io
     _check(load().lisa_td_pipeline_host(
         pipe._h, B, N, len(l), _ints(l), _ints(m), _host(amp), _host(phase), _host(alpha), _host(beta),
         _host(gamma), _host(iota), _host(phi), _host(psi), _host(lam), _host(beta_sky), t0, dt, order,
+        margin_y, generation, margin_lo, margin_hi, C.byref(o), _host(data_spec), _host(weight), kmin,
+        kmax, _host(loglike_out), _host(dh), _host(hh)))
+
+
+def pipeline_host_up2(pipe: Pipeline, B, N, l, m, amp_c, phase_c, alpha_c, beta_c, gamma_c, iota, phi, psi, lam,
+                      beta_sky, t0, dt, order, margin_y, generation, margin_lo, margin_hi, orbit,
+                      data_spec, weight, kmin, kmax, loglike_out, dh=None, hh=None):
+    """mode / angle arrays on the 2 dt grid: [B][M][N/2+1], [B][N/2+1]"""
+    o = make_orbit(orbit)
+    _check(load().lisa_td_pipeline_host_up2(
+        pipe._h, B, N, len(l), _ints(l), _ints(m), _host(amp_c), _host(phase_c), _host(alpha_c), _host(beta_c),
+        _host(gamma_c), _host(iota), _host(phi), _host(psi), _host(lam), _host(beta_sky), t0, dt, order,
         margin_y, generation, margin_lo, margin_hi, C.byref(o), _host(data_spec), _host(weight), kmin,
         kmax, _host(loglike_out), _host(dh), _host(hh)))
 
