@@ -494,7 +494,7 @@ def run_ours(args):
                    "parallelism": f"walker-split x{world}, no collective"},
         "samples_per_s": value * N, "stage_ms": stage_ms, "roofline": roofline, "cpu_baseline": cpu_baseline,
         "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
-            "k1_modes_to_pol_std5": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
+            "k1_modes_to_pol_std5_tma": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
             "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops, "fp64_pipes": pipes,
         "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info,
