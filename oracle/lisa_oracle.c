@@ -32,7 +32,18 @@
  *                            read from tests/golden/
  *   S4  orc_fft_r2c        : naive DFT, numpy.fft, Parseval (C9)
  *   S5  orc_loglike        : closed forms log L(h=d), log L(lambda d), log L(0) (C10)
- *   orbit / PSD            : arm-length and Kepler invariants, independent numpy forms
+ *   orbit                  : arm-length and Kepler invariants, independent numpy forms
+ *   PSD orc_psd_weights    : Eq. 2.15 = the transfer of uncorrelated link / test-mass noises through
+ *                            orc_tdi on static equal arms (sums of squared responses, both
+ *                            generations), Eq. 2.14 at its printed knees and in its power-law limits,
+ *                            zeros of the generation-2 factor (tests/test_oracle_psd_transfer.py)
+ *   C12 second path        : S2 and S3 re-evaluated with absolute-time delays and Neville's recursion
+ *                            in numpy long double, agreement 2e-15 (tests/test_oracle_second_path.py)
+ *   C11 laser residual     : first-order residual sum_terms s Ldot_l D pdot(t - D - L_l) of un-nested
+ *                            TDI on breathing arms, its low-frequency limit and the X2/X1.5 ratio
+ *                            2 omega (L2+L-2+L3+L-3) (tests/test_oracle_laser_residual.py)
+ *   orc_laser_links        : identical to orc_laser_links3 with one laser, and the definition read by
+ *                            orc_delay_read (same file)
  *   orbit TABLE (A21)      : exact on polynomial trajectories, KEPLER1 table vs KEPLER1 closed form
  *   UP  orc_upsample2      : exact on linear series, identity on even samples, closed-form
  *                            midpoint error of a quadratic

@@ -494,10 +494,12 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
       A[q][ks] = (i >= 0 && i < WIN) ? src[i] : 0.0;
     }
   }
+  // cbuf (generic-proxy writes and reads) is about to become y buffer 1 (async-proxy TMA writes):
+  // every thread that touched it fences, THEN the barrier, then one thread issues the copy
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   __syncthreads();  // cbuf is dead from here on: its space becomes the y buffers
 
   // ---- phase 2: stream walkers
-  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // cbuf (generic writes) -> y buffer 1 (TMA writes)
   if (!G::PRIVATE0) prefetch(0, 0);
   for (int c = 0; c < n_chunks; ++c) {
     const int buf = c & 1;
