@@ -18,13 +18,18 @@
  *    lisa_td_plan.  Inputs are never modified.
  *  - Every call only ENQUEUES work on `stream` (a cudaStream_t passed as void*; NULL = the
  *    legacy default stream) and returns without synchronising, except lisa_td_plan_create /
- *    lisa_td_plan_destroy, lisa_td_orbit_table_create, lisa_td_pipeline_host and the lisa_td_probe_*
- *    calls, which synchronise.  The enqueue-only calls may therefore be captured into a CUDA graph
- *    and replayed (tests/test_gpu_graph.py; call lisa_td_loglike once with the batch size before
+ *    lisa_td_plan_destroy, lisa_td_orbit_table_create, lisa_td_pipeline_host and lisa_td_check,
+ *    which synchronise.  The enqueue-only calls may therefore be captured into a CUDA graph and
+ *    replayed (tests/test_gpu_graph.py; call lisa_td_loglike once with the batch size before
  *    capturing: the first use of a batch size creates its cuFFT plan).
  *  - Return value: LISA_TD_OK (0) or a negative lisa_td_status.  Argument errors are detected
  *    on the host before any launch.  The library never throws, aborts or falls back to the
  *    CPU.  lisa_td_last_error() returns a thread-local description of the last failure.
+ *  - Device-side range checks.  Tile and window sizes of S2 / S3 follow from host-side bounds on the
+ *    orbit (max |r|, max L, drift of the common delay; for a TABLE orbit taken from its nodes).  A
+ *    kernel that meets a delay outside those bounds does not clamp silently: it raises a sticky
+ *    flag, and the next lisa_td_check / lisa_td_pipeline_host returns LISA_TD_EINVAL (the outputs
+ *    written since the previous check are then invalid).
  *  - Walkers b = 0..B-1, samples n = 0..N-1 at t_n = t0 + n*dt, `order` p odd in [1,63]
  *    (p+1 Lagrange taps; p = 1 is the paper's linear interpolation).
  *  - Link order everywhere: l = [1,2,3,-1,-2,-3] <-> (sender,receiver) =
@@ -58,6 +63,11 @@ typedef enum {
 
 LISA_TD_API const char* lisa_td_last_error(void);
 LISA_TD_API int lisa_td_version(void);
+
+/* Synchronises `stream` and reports (then clears) the device-side range checks raised by the
+ * kernels since the last check: LISA_TD_OK, LISA_TD_EINVAL (see "Device-side range checks" above)
+ * or LISA_TD_ECUDA if the stream itself failed. */
+LISA_TD_API int lisa_td_check(void* stream);
 
 /* Orbit description (host struct, copied at call time).
  * kind 0 = STATIC : spacecraft positions r_static[spacecraft][xyz] in metres and the six light
@@ -106,6 +116,8 @@ LISA_TD_API int lisa_td_orbit_table_destroy(lisa_td_orbit_table* table);
  *   h_k = amp_k e^{-i phase_k},  R = R(alpha,beta,gamma)(t) . R(euler0) . R(phi, iota, 0)
  * l_host/m_host: n_modes (<= 16) mode labels, 2 <= l <= 8, 0 <= m <= l (the -m partner is implied).
  * amp, phase: [B][n_modes][N].  alpha,beta,gamma: [B][N] each, or all three NULL (aligned spin).
+ * |phase|, |alpha|, |gamma| must stay below 2^30 rad (1e9): the kernels reduce arguments with a
+ * two-constant Cody-Waite step that is good to 6e-17 up to there (a months-long chirp reaches 1e6).
  * iota, phi, psi: [B].  euler0: [B][3] constant J->L0 angles or NULL.  hplus, hcross: [B][N]. */
 LISA_TD_API int lisa_td_modes_to_pol(int B, long long N, int n_modes, const int* l_host, const int* m_host,
                          const double* amp, const double* phase, const double* alpha,
@@ -148,13 +160,20 @@ LISA_TD_API int lisa_td_laser_links(long long N, double t0, double dt, int order
  * fractional-delay read of one y series at D = (sum of the listed L_l(t_n))/dt (A10: summed, all
  * L at the output time).  y: [B][6][N].  tdi: [B][3][N], out_kind 0 = X,Y,Z, 1 = A,E,T; samples
  * outside [margin_lo, N - margin_hi) are exact zeros.  Requires margin_lo >= ceil(7 Lmax/dt) +
- * (p+1)/2 (3 Lmax for generation 15) and margin_hi >= (p+1)/2. */
+ * (p+1)/2 (3 Lmax for generation 15) and margin_hi >= (p+1)/2.  If y came from
+ * lisa_td_link_response with margin_y, the caller must ADD margin_y to both (reading A7: TDI must
+ * not interpolate across the zeroed edge of y); this call cannot know margin_y and does not check
+ * that, lisa_td_response_tdi and lisa_td_pipeline_host do. */
 LISA_TD_API int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
                  long long margin_lo, long long margin_hi, const double* y,
                  const lisa_td_orbit* orbit_host, double* tdi, void* stream);
 
-/* S2+S3 in one call: h+,hx -> tdi.  The six links of a walker chunk live in `workspace`
- * (device, >= lisa_td_response_tdi_workspace_bytes(B,N) bytes), never in a caller array. */
+/* S2+S3 in one call: h+,hx -> tdi.  This is lisa_td_link_response into `workspace` followed by
+ * lisa_td_tdi2 from it: all six links of all B walkers make one round trip through HBM ([B][6][N]
+ * doubles = 48 B N bytes, the size lisa_td_response_tdi_workspace_bytes returns), they just never
+ * appear in a caller array.  An on-chip fusion was prototyped and measured slower (DESIGN.md
+ * section 9, profiles/r2_fused_prototype.md): both kernels are bound by fp64 arithmetic, not by the
+ * round trip.  Requires margin_lo >= margin_y + reach and margin_hi >= margin_y + (p+1)/2. */
 LISA_TD_API long long lisa_td_response_tdi_workspace_bytes(int B, long long N);
 LISA_TD_API int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, long long margin_y,
                          int generation, int out_kind, long long margin_lo, long long margin_hi,
@@ -162,8 +181,9 @@ LISA_TD_API int lisa_td_response_tdi(int B, long long N, double t0, double dt, i
                          const double* beta_sky, const lisa_td_orbit* orbit_host, double* tdi,
                          void* workspace, long long workspace_bytes, void* stream);
 
-/* S4+S5 plan: owns the cuFFT plan (batched real-to-complex, length N), the spectrum scratch
- * and the partial-sum scratch for up to B walkers. */
+/* S4+S5 plan: owns the cuFFT plans (batched complex-to-complex of length N/2 on the packed real
+ * series, one per batch size seen, at most 8, sharing one work area), the spectrum scratch and the
+ * partial-sum scratch for up to B walkers.  Not thread-safe: one host thread per plan at a time. */
 typedef struct lisa_td_plan lisa_td_plan;
 LISA_TD_API int lisa_td_plan_create(lisa_td_plan** out, int B, long long N);
 LISA_TD_API int lisa_td_plan_destroy(lisa_td_plan* plan);
@@ -244,27 +264,6 @@ LISA_TD_API int lisa_td_pipeline_host_up2(lisa_td_pipeline* p, int B, long long 
                               const lisa_td_orbit* orbit_host, const double* data_spec_host,
                               const double* weight_host, long long kmin, long long kmax,
                               double* loglike_host, double* dh_host, double* hh_host);
-
-/* Measurement support: a register-resident chain of `iters` x 8 dependent-free DFMA per thread on
- * `blocks` x `threads`; returns the elapsed milliseconds (CUDA events) in *ms_host and writes one
- * double per thread to sink (device, blocks*threads doubles) so the work is not optimised away.
- * FLOP count = 2 * 8 * iters * blocks * threads. */
-LISA_TD_API int lisa_td_probe_dfma(long long iters, int blocks, int threads, double* sink, float* ms_host,
-                       void* stream);
-
-/* Measurement support: in every block, dfma_warps warps run 8 independent DFMA chains per thread and
- * dmma_warps warps run 4 independent mma.sync.m8n8k4.f64 accumulator pairs, `iters` rounds each
- * (dfma_warps + dmma_warps <= 32).  FLOP count = 2 * iters * blocks * (256 * dfma_warps + 1024 *
- * dmma_warps).  Answers whether the fp64 tensor path (K3) and the DFMA pipe (K1, K2) are separate
- * units: on B200 the times add, i.e. they are one resource.  sink: blocks * 32 * (dfma_warps +
- * dmma_warps) doubles. */
-LISA_TD_API int lisa_td_probe_fp64_pipes(long long iters, int blocks, int dfma_warps, int dmma_warps, double* sink,
-                             float* ms_host, void* stream);
-
-/* Testing switch: 1 routes S1/S2/S3 through the generic (any mode list, runtime-order, unmerged)
- * kernels even where a specialised instantiation exists, so the tests can cover both; 2 keeps the
- * specialised kernels but routes the five-mode S1 through its non-TMA variant; 0 = normal. */
-LISA_TD_API void lisa_td_debug_force_generic(int on);
 
 #ifdef __cplusplus
 }

@@ -13,6 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "liblisa_td.so")
+PROBE_LIB = os.path.join(HERE, "liblisa_td_probe.so")  # bench-only fp64 probes (csrc/probe.cu), not product ABI
 SOURCES = ["api.cu", "k1_modes_to_pol.cu", "k2_link_response.cu", "k3_tdi.cu", "k5_loglike.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(ROOT, "include", "lisa_td.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -43,6 +44,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [NVCC, "-shared", "-o", LIB, *objs, "-L/usr/local/cuda/lib64", "-lcufft",
                "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
         subprocess.run(cmd, check=True)
+    probe_src = os.path.join(CSRC, "probe.cu")
+    if force or _stale(PROBE_LIB, [probe_src, os.path.join(CSRC, "lisa_td_probe.h")]):
+        subprocess.run([NVCC, *FLAGS, "-shared", probe_src, "-o", PROBE_LIB], check=True)
     return LIB
 
 

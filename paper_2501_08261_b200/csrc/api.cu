@@ -5,6 +5,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -27,6 +28,59 @@ int check_cuda(cudaError_t e, const char* what) {
   if (e == cudaSuccess) return LISA_TD_OK;
   return set_error(e == cudaErrorMemoryAllocation ? LISA_TD_ENOMEM : LISA_TD_ECUDA, "%s: %s (%s)", what,
                    cudaGetErrorString(e), cudaGetErrorName(e));
+}
+
+int sm_count() {
+  static thread_local int cached_dev = -1, cached = 0;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+  if (dev != cached_dev) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    cached_dev = dev;
+    cached = n;
+  }
+  return cached;
+}
+
+// ------------------------------------------------------------------ sticky device-side errors
+unsigned int* device_error_words() {
+  static unsigned int* words = nullptr;
+  static bool tried = false;
+  if (!tried) {  // benign race: two first calls from two threads would leak 16 bytes of pinned memory
+    tried = true;
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, DEVERR_COUNT * sizeof(unsigned int), cudaHostAllocMapped | cudaHostAllocPortable) == cudaSuccess) {
+      memset(p, 0, DEVERR_COUNT * sizeof(unsigned int));
+      words = static_cast<unsigned int*>(p);
+    } else {
+      cudaGetLastError();
+    }
+  }
+  return words;
+}
+// Call after a synchronisation: reports and clears what the kernels raised since the last check.
+int take_device_errors(const char* fn) {
+  volatile unsigned int* w = device_error_words();
+  if (!w) return LISA_TD_OK;
+  const unsigned k2 = w[DEVERR_K2_WINDOW], k3 = w[DEVERR_K3_WINDOW], la = w[DEVERR_LASER_WINDOW];
+  if (!(k2 | k3 | la)) return LISA_TD_OK;
+  w[DEVERR_K2_WINDOW] = w[DEVERR_K3_WINDOW] = w[DEVERR_LASER_WINDOW] = 0;
+  return set_error(LISA_TD_EINVAL,
+                   "%s: a kernel found a delay outside the range the host-side orbit bounds promised (%s%s%s): "
+                   "the outputs written since the last check are invalid (orbit far from the bounds of its "
+                   "description, e.g. a TABLE orbit whose arms or centroid move faster than its nodes suggest)",
+                   fn, k2 ? "link-response strain window " : "", k3 ? "TDI stencil window " : "",
+                   la ? "laser-link window" : "");
+}
+
+// Test-only dispatch switch, read from the environment at every call (NOT part of the ABI):
+// LISA_TD_DISPATCH=1 routes S1/S2/S3 through the generic (any mode list, runtime-order, unmerged)
+// kernels even where a specialised instantiation exists, 2 keeps the specialised kernels but
+// routes the five-mode S1 through its non-TMA variant; unset or 0 = normal.
+int dispatch_mode() {
+  const char* e = getenv("LISA_TD_DISPATCH");
+  return e ? atoi(e) : 0;
 }
 
 // ------------------------------------------------------------------ constant tables
@@ -229,7 +283,8 @@ int run_link_response(int, long long, double, double, int, long long, const doub
 int run_laser_links(long long, double, double, int, long long, const double*, const OrbitDev&,
                     double*, cudaStream_t);
 int run_tdi(int, long long, double, double, int, int, int, long long, long long, const double*,
-            const OrbitDev&, double*, cudaStream_t);
+            const OrbitDev&, double*, cudaStream_t, double* tab_ws = nullptr, long long tab_ws_bytes = 0);
+long long tdi_workspace_bytes(long long N);
 struct Plan;
 int plan_create(Plan**, int, long long);
 int plan_destroy(Plan*);
@@ -238,8 +293,6 @@ int run_loglike(Plan*, int, long long, const double*, const double*, const doubl
                 long long, double*, double*, double*, cudaStream_t, int n_ch);
 int run_fisher(Plan*, int, long long, const double*, const double*, const double*, long long, long long,
                double*, cudaStream_t);
-extern int g_force_generic;
-extern int g_k1_no_tma;
 
 // ------------------------------------------------------------------ validation helpers
 static int check_common(const char* fn, int B, long long N, double dt, int order) {
@@ -269,16 +322,21 @@ static int check_margin_y(const char* fn, long long N, double dt, int order, lon
   if (N < 2 * margin_y) return set_error(LISA_TD_EINVAL, "%s: N=%lld must be >= 2*margin_y", fn, N);
   return LISA_TD_OK;
 }
+// margin_y: the margin of the link responses that feed this TDI call when the library knows it (the
+// combined entry points), 0 otherwise: TDI must not interpolate across the hard-zeroed edge of y
+// (reading A7: m_lo >= m_y + reach, m_hi >= m_y + (p+1)/2).
 static int check_margin_tdi(const char* fn, long long N, double dt, int order, int generation,
-                            long long margin_lo, long long margin_hi, const OrbitDev& od) {
+                            long long margin_lo, long long margin_hi, const OrbitDev& od, long long margin_y = 0) {
   if (generation != 15 && generation != 20)
     return set_error(LISA_TD_EINVAL, "%s: generation must be 15 or 20 (got %d)", fn, generation);
   const int h = (order + 1) / 2;
-  const long long need_lo = (long long)ceil((generation == 20 ? 7 : 3) * od.max_L / dt) + h;
+  const long long need_lo = margin_y + (long long)ceil((generation == 20 ? 7 : 3) * od.max_L / dt) + h;
   if (margin_lo < need_lo)
-    return set_error(LISA_TD_EINVAL, "%s: margin_lo=%lld does not cover the stencil reach %lld", fn, margin_lo, need_lo);
-  if (margin_hi < h)
-    return set_error(LISA_TD_EINVAL, "%s: margin_hi=%lld must be >= (order+1)/2 = %d", fn, margin_hi, h);
+    return set_error(LISA_TD_EINVAL, "%s: margin_lo=%lld does not cover margin_y=%lld plus the stencil reach (need %lld)", fn,
+                     margin_lo, margin_y, need_lo);
+  if (margin_hi < margin_y + h)
+    return set_error(LISA_TD_EINVAL, "%s: margin_hi=%lld must be >= margin_y + (order+1)/2 = %lld", fn, margin_hi,
+                     margin_y + h);
   if (N < margin_lo + margin_hi) return set_error(LISA_TD_EINVAL, "%s: N=%lld smaller than the margins", fn, N);
   return LISA_TD_OK;
 }
@@ -348,9 +406,10 @@ int lisa_td_orbit_table_destroy(lisa_td_orbit_table* t) {
   return LISA_TD_OK;
 }
 int lisa_td_version(void) { return 100; }
-void lisa_td_debug_force_generic(int on) {
-  g_force_generic = on == 1;
-  g_k1_no_tma = on == 2;
+int lisa_td_check(void* stream) {
+  const char* fn = "lisa_td_check";
+  LISA_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return take_device_errors(fn);
 }
 
 int lisa_td_modes_to_pol(int B, long long N, int n_modes, const int* l_host, const int* m_host,
@@ -441,9 +500,11 @@ int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int genera
                  (cudaStream_t)stream);
 }
 
+// [B][6][N] link responses, then the anchor tables of S3 (k3_tdi.cu)
+static long long links_bytes(int B, long long N) { return ((long long)sizeof(double) * 6 * (long long)B * N + 255) / 256 * 256; }
 long long lisa_td_response_tdi_workspace_bytes(int B, long long N) {
   if (B <= 0 || N <= 0) return 0;
-  return (long long)sizeof(double) * 6 * (long long)B * N;
+  return links_bytes(B, N) + tdi_workspace_bytes(N);
 }
 
 int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, long long margin_y,
@@ -464,13 +525,14 @@ int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, lo
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
   if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
-  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od, margin_y))) return rc;
   double* y = static_cast<double*>(workspace);
   if ((rc = run_link_response(B, N, t0, dt, order, margin_y, hplus, hcross, lambda, beta_sky, od, y,
                               (cudaStream_t)stream)))
     return rc;
   return run_tdi(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi,
-                 (cudaStream_t)stream);
+                 (cudaStream_t)stream, reinterpret_cast<double*>(static_cast<char*>(workspace) + links_bytes(B, N)),
+                 tdi_workspace_bytes(N));
 }
 
 struct lisa_td_plan {
@@ -565,7 +627,8 @@ int lisa_td_psd_weights(long long N, double dt, double acc_noise, double oms_noi
     // Eq. 2.15 with x = 2 pi f L/c (A14)
     const double x = om * arm_s, sx = sin(x), cx = cos(x), sh = sin(0.5 * x);
     double s_ae = 8 * sx * sx * (2 * s_acc * (3 + 2 * cx + cos(2 * x)) + s_op * (2 + cx));
-    double s_t = 16 * s_op * (1 - cx) * sx * sx + 128 * s_acc * sx * sx * sh * sh * sh * sh;
+    // 1 - cos x written as 2 sin^2(x/2): no cancellation at low frequency
+    double s_t = 16 * s_op * (2 * sh * sh) * sx * sx + 128 * s_acc * sx * sx * sh * sh * sh * sh;
     if (generation == 20) {
       const double g = 4 * sin(2 * x) * sin(2 * x);
       s_ae *= g;
@@ -587,6 +650,7 @@ struct lisa_td_pipeline {
   cudaEvent_t copied[2], done[2];
   double* in[2];      // per buffer: amp, phase [cB][M][N], (alpha,beta,gamma [cB][N]), 5 scalars [cB]
   double *hp, *hc, *y, *tdi, *ll;  // ll: [3][cB] (loglike, dh, hh)
+  double* tab;                     // anchor tables of S3
   double *data_spec, *weight;
   lisa::Plan* plan;
   size_t in_doubles;
@@ -599,7 +663,7 @@ int lisa_td_pipeline_destroy(lisa_td_pipeline* p) {
     if (p->copied[i]) cudaEventDestroy(p->copied[i]);
     if (p->done[i]) cudaEventDestroy(p->done[i]);
   }
-  cudaFree(p->hp); cudaFree(p->hc); cudaFree(p->y); cudaFree(p->tdi); cudaFree(p->ll);
+  cudaFree(p->hp); cudaFree(p->hc); cudaFree(p->y); cudaFree(p->tdi); cudaFree(p->ll); cudaFree(p->tab);
   cudaFree(p->data_spec); cudaFree(p->weight);
   if (p->plan) plan_destroy(p->plan);
   if (p->s_copy) cudaStreamDestroy(p->s_copy);
@@ -630,6 +694,7 @@ int lisa_td_pipeline_create(lisa_td_pipeline** out, int chunk_B, long long N, in
   PIPE_TRY(cudaMalloc(&p->hc, sizeof(double) * cB * N));
   PIPE_TRY(cudaMalloc(&p->y, sizeof(double) * cB * 6 * N));
   PIPE_TRY(cudaMalloc(&p->tdi, sizeof(double) * cB * 3 * N));
+  PIPE_TRY(cudaMalloc(&p->tab, (size_t)tdi_workspace_bytes(N)));
   PIPE_TRY(cudaMalloc(&p->ll, sizeof(double) * (4 * cB + 8)));
   PIPE_TRY(cudaMalloc(&p->data_spec, sizeof(double) * 6 * p->nf));
   PIPE_TRY(cudaMalloc(&p->weight, sizeof(double) * 4 * p->nf));
@@ -671,13 +736,16 @@ static int pipeline_run(const char* fn, int up2, lisa_td_pipeline* p, int B, lon
   if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
   if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
   if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
-  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od, margin_y))) return rc;
 
   const size_t M = n_modes, cB = p->chunk_B;
   // up2 (reading A20): the mode and angle arrays live on the 2 dt grid, Nin = N/2 + 1 samples
   // per row; sub-arrays start on even offsets so that every device array stays 16-byte aligned
   const size_t Nin = up2 ? (size_t)(N / 2 + 1) : (size_t)N;
   auto even = [](size_t v) { return (v + 1) & ~(size_t)1; };
+  // everything that enqueues work runs inside `enqueue`, so that a failure half way can still wait for
+  // what is already in flight before returning: the caller may free its host buffers right after
+  auto enqueue = [&]() -> int {
   LISA_CUDA(cudaMemcpyAsync(p->data_spec, data_spec_host, sizeof(double) * 6 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
   LISA_CUDA(cudaMemcpyAsync(p->weight, weight_host, sizeof(double) * 3 * p->nf, cudaMemcpyHostToDevice, p->s_copy));
   int it = 0;
@@ -717,7 +785,8 @@ static int pipeline_run(const char* fn, int up2, lisa_td_pipeline* p, int B, lon
     if ((rc = run_link_response((int)nb, N, t0, dt, order, margin_y, p->hp, p->hc, d_sc + 3 * sc_stride,
                                 d_sc + 4 * sc_stride, od, p->y, p->s_comp, up2)))
       return rc;
-    if ((rc = run_tdi((int)nb, N, t0, dt, order, generation, 1, margin_lo, margin_hi, p->y, od, p->tdi, p->s_comp)))
+    if ((rc = run_tdi((int)nb, N, t0, dt, order, generation, 1, margin_lo, margin_hi, p->y, od, p->tdi, p->s_comp, p->tab,
+                      tdi_workspace_bytes(N))))
       return rc;
     if ((rc = run_loglike(p->plan, (int)nb, N, p->tdi, p->data_spec, p->weight, kmin, kmax, p->ll, p->ll + sc_stride,
                           p->ll + 2 * sc_stride, p->s_comp, 3)))
@@ -727,9 +796,14 @@ static int pipeline_run(const char* fn, int up2, lisa_td_pipeline* p, int B, lon
     if (hh_host) LISA_CUDA(cudaMemcpyAsync(hh_host + b0, p->ll + 2 * sc_stride, sizeof(double) * nb, cudaMemcpyDeviceToHost, p->s_comp));
     LISA_CUDA(cudaEventRecord(p->done[buf], p->s_comp));
   }
-  LISA_CUDA(cudaStreamSynchronize(p->s_copy));
-  LISA_CUDA(cudaStreamSynchronize(p->s_comp));
   return LISA_TD_OK;
+  };
+  rc = enqueue();
+  const cudaError_t e1 = cudaStreamSynchronize(p->s_copy), e2 = cudaStreamSynchronize(p->s_comp);
+  if (rc) return rc;  // the first failure, reported after both streams have drained
+  LISA_CUDA(e1);
+  LISA_CUDA(e2);
+  return take_device_errors(fn);
 }
 
 int lisa_td_pipeline_host(lisa_td_pipeline* p, int B, long long N, int n_modes, const int* l_host,
@@ -764,85 +838,6 @@ int lisa_td_pipeline_host_up2(lisa_td_pipeline* p, int B, long long N, int n_mod
                       beta_host, gamma_host, iota_host, phi_host, psi_host, lambda_host, beta_sky_host, t0, dt, order,
                       margin_y, generation, margin_lo, margin_hi, orbit_host, data_spec_host, weight_host, kmin, kmax,
                       loglike_host, dh_host, hh_host);
-}
-
-// ---------------------------------------------------------------------- DFMA probe
-__global__ void k_probe_dfma(long long iters, double* sink) {
-  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3;
-  double a4 = a0 + 4e-3, a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
-  const double m = 0.999999, c = 1e-7;
-  for (long long i = 0; i < iters; ++i) {
-    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-  }
-  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-}
-
-// Warps 0..dfma_warps-1 of every block run 8 independent DFMA chains per thread, the next dmma_warps
-// warps run 4 independent DMMA (mma.sync m8n8k4 f64) accumulator pairs: do the two paths share a pipe?
-__global__ void __launch_bounds__(1024) k_probe_fp64_pipes(long long iters, int dfma_warps, int dmma_warps, double* sink) {
-  const int wid = threadIdx.x >> 5;
-  const double x = 1.0 + threadIdx.x * 1e-9, y = 0.999999;
-  double r = 0.0;
-  if (wid < dfma_warps) {
-    double a0 = x, a1 = x + 1e-3, a2 = x + 2e-3, a3 = x + 3e-3, a4 = x + 4e-3, a5 = x + 5e-3, a6 = x + 6e-3, a7 = x + 7e-3;
-    for (long long i = 0; i < iters; ++i) {
-      a0 = fma(a0, y, x); a1 = fma(a1, y, x); a2 = fma(a2, y, x); a3 = fma(a3, y, x);
-      a4 = fma(a4, y, x); a5 = fma(a5, y, x); a6 = fma(a6, y, x); a7 = fma(a7, y, x);
-    }
-    r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-  } else {
-    double d[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    for (long long i = 0; i < iters; ++i) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                     : "+d"(d[2 * q]), "+d"(d[2 * q + 1])
-                     : "d"(x), "d"(y));
-    }
-    r = ((d[0] + d[1]) + (d[2] + d[3])) + ((d[4] + d[5]) + (d[6] + d[7]));
-  }
-  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = r;
-}
-
-int lisa_td_probe_fp64_pipes(long long iters, int blocks, int dfma_warps, int dmma_warps, double* sink, float* ms_host,
-                             void* stream) {
-  const char* fn = "lisa_td_probe_fp64_pipes";
-  if (iters <= 0 || blocks <= 0 || dfma_warps < 0 || dmma_warps < 0 || dfma_warps + dmma_warps < 1 ||
-      dfma_warps + dmma_warps > 32 || !sink || !ms_host)
-    return set_error(LISA_TD_EINVAL, "%s: bad arguments", fn);
-  cudaStream_t st = (cudaStream_t)stream;
-  cudaEvent_t e0, e1;
-  LISA_CUDA(cudaEventCreate(&e0));
-  LISA_CUDA(cudaEventCreate(&e1));
-  LISA_CUDA(cudaEventRecord(e0, st));
-  k_probe_fp64_pipes<<<blocks, 32 * (dfma_warps + dmma_warps), 0, st>>>(iters, dfma_warps, dmma_warps, sink);
-  LISA_CUDA(cudaPeekAtLastError());
-  LISA_CUDA(cudaEventRecord(e1, st));
-  LISA_CUDA(cudaEventSynchronize(e1));
-  LISA_CUDA(cudaEventElapsedTime(ms_host, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  return LISA_TD_OK;
-}
-
-int lisa_td_probe_dfma(long long iters, int blocks, int threads, double* sink, float* ms_host, void* stream) {
-  const char* fn = "lisa_td_probe_dfma";
-  if (iters <= 0 || blocks <= 0 || threads <= 0 || threads > 1024 || !sink || !ms_host)
-    return set_error(LISA_TD_EINVAL, "%s: bad arguments", fn);
-  cudaStream_t st = (cudaStream_t)stream;
-  cudaEvent_t e0, e1;
-  LISA_CUDA(cudaEventCreate(&e0));
-  LISA_CUDA(cudaEventCreate(&e1));
-  LISA_CUDA(cudaEventRecord(e0, st));
-  k_probe_dfma<<<blocks, threads, 0, st>>>(iters, sink);
-  LISA_CUDA(cudaPeekAtLastError());
-  LISA_CUDA(cudaEventRecord(e1, st));
-  LISA_CUDA(cudaEventSynchronize(e1));
-  LISA_CUDA(cudaEventElapsedTime(ms_host, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  return LISA_TD_OK;
 }
 
 }  // extern "C"

@@ -24,6 +24,20 @@ int check_cuda(cudaError_t e, const char* what);
 #define LISA_LAUNCH_CHECK(name) LISA_CUDA(cudaPeekAtLastError())
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+int sm_count();  // multiprocessors of the current device (api.cu)
+
+// ------------------------------------------------------------------ sticky device-side errors
+// The kernels size their shared-memory tiles and merged stencil windows from HOST-side bounds on
+// the orbit (max |r|, max L, drift of the common delay).  Where an index computed on the device
+// falls outside what those bounds promised, the kernel sets one of these words (and clamps the
+// index for memory safety only): the result is then wrong, and the next synchronising call
+// (lisa_td_check, lisa_td_pipeline_host) returns LISA_TD_EINVAL instead of a silent wrong answer.
+// The words live in mapped pinned host memory (one allocation per process, host pointer ==
+// device pointer under unified addressing), so reading them costs no copy.
+enum DevErr { DEVERR_K2_WINDOW = 0, DEVERR_K3_WINDOW = 1, DEVERR_LASER_WINDOW = 2, DEVERR_COUNT = 4 };
+unsigned int* device_error_words();  // api.cu; NULL if the allocation failed (checks are then skipped)
+int take_device_errors(const char* fn);  // after a synchronisation: LISA_TD_EINVAL if a word is set (and clears it)
+int dispatch_mode();  // test-only: environment variable LISA_TD_DISPATCH (0 normal, 1 generic kernels, 2 S1 without TMA)
 
 constexpr double C_LIGHT = 299792458.0;  // m/s
 constexpr int MAX_HALF = 32;             // (p+1)/2 for p <= 63
@@ -80,6 +94,10 @@ struct OrbitDev {
 int make_orbit_dev(const lisa_td_orbit* o, OrbitDev* out);
 
 #ifdef __CUDACC__
+
+__device__ __forceinline__ void raise_error(unsigned int* words, int which) {
+  if (words) reinterpret_cast<volatile unsigned int*>(words)[which] = 1u;
+}
 
 // Link index 0..5 <-> l = [1,2,3,-1,-2,-3]; sender / receiver spacecraft (0-based).
 __host__ __device__ constexpr int link_s(int l) { return l < 3 ? (l + 2) % 3 : (l - 3 + 1) % 3; }
@@ -264,115 +282,14 @@ __device__ __forceinline__ void orbit_arm_times(const OrbitDev& o, double t, dou
 }
 
 // ------------------------------------------------------------------ Lagrange stencil
-// HT > 0: half-width known at compile time (fully unrolled, prefix products in registers).
-// HT = 0: runtime half-width Hrt <= MAX_HALF (prefix products in local memory).
+// Array-free ("Horner in node pairs") form of the interpolant.  With the scaled pair factors of
+// LagS, Q'_k = rho_k (q + k(1-k)), q = eps (eps - 1), prefix P_k = g prod_{i<k} Q'_i and
+//   v_k = (eps+k-1) x_k + (k-eps) x_{1-k},
+// the sum  sum_k P_k (prod_{i>k} Q'_i) v_k  is the end value of  T_k = Q'_k T_{k-1} + P_k v_k,
+// T_0 = 0:  no prefix array, no suffix chain, 11 fp64 ops per node pair for two series, and so
+// few live registers that the tap loads can be issued far ahead of their use.
+// HT > 0: half-width known at compile time (fully unrolled); HT = 0: runtime half-width Hrt.
 //
-// lagrange_coeffs: c[j + H - 1] = c_j(eps), j = -H+1..H.   ~9 fp64 ops per node pair.
-template <int HT>
-__device__ __forceinline__ void lagrange_coeffs(double eps, int Hrt, const LagW& lw,
-                                                double* __restrict__ c) {
-  const int H = HT > 0 ? HT : Hrt;
-  double P[HT > 0 ? HT + 1 : MAX_HALF + 1];
-  const double q = eps * (eps - 1.0);
-  P[1] = 1.0;
-#pragma unroll
-  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
-  double S = 1.0;
-#pragma unroll
-  for (int k = H; k >= 1; --k) {
-    double a = (lw.w[k - 1] * P[k]) * S;
-    c[k + H - 1] = a * (eps + (double)(k - 1));
-    c[H - k] = a * ((double)k - eps);
-    S *= q + (double)(k * (1 - k));
-  }
-}
-
-// Fused coefficient sweep + dot product with an interleaved (h+, hx) series:
-// x points at tap j = 0, i.e. x[j] is read for j = -H+1..H.
-template <int HT>
-__device__ __forceinline__ void lagrange_dot2(double eps, int Hrt, const LagW& lw,
-                                              const double2* __restrict__ x, double& sp,
-                                              double& sc) {
-  const int H = HT > 0 ? HT : Hrt;
-  double P[HT > 0 ? HT + 1 : MAX_HALF + 1];
-  const double q = eps * (eps - 1.0);
-  P[1] = 1.0;
-#pragma unroll
-  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * (q + (double)(k * (1 - k)));
-  double S = 1.0, ap = 0.0, ac = 0.0, bp = 0.0, bc = 0.0;
-#pragma unroll
-  for (int k = H; k >= 1; --k) {
-    double a = (lw.w[k - 1] * P[k]) * S;
-    double ck = a * (eps + (double)(k - 1));
-    double cm = a * ((double)k - eps);
-    double2 xk = x[k], xm = x[1 - k];
-    ap = fma(ck, xk.x, ap);
-    ac = fma(ck, xk.y, ac);
-    bp = fma(cm, xm.x, bp);
-    bc = fma(cm, xm.y, bc);
-    S *= q + (double)(k * (1 - k));
-  }
-  sp = ap + bp;
-  sc = ac + bc;
-}
-
-// Compile-time half-width H, scaled weights (LagS): coefficient sweep + two dot products in
-// 7 + 4 fp64 ops per node pair.  c_k = a_k (eps + k - 1) = fma(a_k, k-1, a_k eps),
-// c_{1-k} = a_k (k - eps) = fma(a_k, k, -a_k eps).
-template <int H>
-__device__ __forceinline__ void lagrange_dot2s(double eps, const LagS& ls,
-                                               const double2* __restrict__ x, double& sp,
-                                               double& sc) {
-  double P[H + 1];
-  const double q = eps * (eps - 1.0);
-  P[1] = ls.g;
-#pragma unroll
-  for (int k = 1; k < H; ++k) P[k + 1] = P[k] * fma(ls.rho[k - 1], q, ls.rc[k - 1]);
-  double S = 1.0, ap = 0.0, ac = 0.0, bp = 0.0, bc = 0.0;
-#pragma unroll
-  for (int k = H; k >= 1; --k) {
-    const double a = P[k] * S;
-    const double t = a * eps;
-    const double ck = fma(a, (double)(k - 1), t);
-    const double cm = fma(a, (double)k, -t);
-    const double2 xk = x[k], xm = x[1 - k];
-    ap = fma(ck, xk.x, ap);
-    ac = fma(ck, xk.y, ac);
-    bp = fma(cm, xm.x, bp);
-    bc = fma(cm, xm.y, bc);
-    if (k > 1) S *= fma(ls.rho[k - 1], q, ls.rc[k - 1]);
-  }
-  sp = ap + bp;
-  sc = ac + bc;
-}
-
-// Array-free ("Horner in node pairs") form of the same sum.  With S_k = prod_{i>k} Q'_i,
-//   sum_k P_k S_k v_k,  v_k = (eps+k-1) x_k + (k-eps) x_{1-k},
-// is the end value of  T_k = Q'_k T_{k-1} + P_k v_k,  T_0 = 0:  no prefix array, no suffix
-// chain, 11 fp64 ops per node pair for two series, and so few live registers that the tap
-// loads can be issued far ahead of their use.  HT > 0: unrolled; HT = 0: runtime half-width.
-template <int HT>
-__device__ __forceinline__ void lagrange_dot2h(double eps, int Hrt, const LagS& ls,
-                                               const double2* __restrict__ x, double& sp,
-                                               double& sc) {
-  const int H = HT > 0 ? HT : Hrt;
-  const double q = eps * (eps - 1.0);
-  double P = ls.g, Tp = 0.0, Tc = 0.0;
-#pragma unroll
-  for (int k = 1; k <= H; ++k) {
-    const double Q = fma(ls.rho[k - 1], q, ls.rc[k - 1]);
-    const double t = P * eps;
-    const double ck = k == 1 ? t : fma(P, (double)(k - 1), t);
-    const double cm = fma(P, (double)k, -t);
-    const double2 xk = x[k], xm = x[1 - k];
-    Tp = fma(Tp, Q, fma(ck, xk.x, cm * xm.x));
-    Tc = fma(Tc, Q, fma(ck, xk.y, cm * xm.y));
-    P *= Q;
-  }
-  sp = Tp;
-  sc = Tc;
-}
-
 // Two ADJACENT output samples a, b = a+1 with the same integer delay: their windows are
 // x[e+1-H .. e+H] and x[e+2-H .. e+H+1], so one pass loads 2H+1 taps for both instead of 4H.
 // The series is stored split by parity of the element index (xe[i] = x[2i], xo[i] = x[2i+1])

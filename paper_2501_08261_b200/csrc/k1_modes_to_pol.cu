@@ -444,8 +444,6 @@ static long double binom_ld(int n, int k) {
   return r;
 }
 
-extern int g_force_generic;
-int g_k1_no_tma = 0;  // debug switch (lisa_td_debug_force_generic(2)): the load-everything-first five-mode kernel
 
 int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m, const double* amp,
                      const double* phase, const double* alpha, const double* beta,
@@ -456,7 +454,7 @@ int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m
   {
     static const int SL[5] = {2, 2, 3, 4, 5}, SM[5] = {2, 1, 3, 4, 5};
     K1FastParams f;
-    bool ok = !g_force_generic;
+    bool ok = dispatch_mode() != 1;
     for (int j = 0; j < 5; ++j) f.idx[j] = -1;
     for (int k = 0; k < n_modes && ok; ++k) {
       int j = 0;
@@ -475,7 +473,7 @@ int run_modes_to_pol(int B, long long N, int n_modes, const int* l, const int* m
       f.B = B; f.N = N; f.n_modes = n_modes; f.twisted = alpha != nullptr; f.have_e0 = euler0 != nullptr;
       f.amp = amp; f.phase = phase; f.alpha = alpha; f.beta = beta; f.gamma = gamma;
       f.iota = iota; f.phi = phi; f.psi = psi; f.euler0 = euler0; f.hplus = hplus; f.hcross = hcross;
-      if ((N & 1) == 0 && !g_k1_no_tma) {
+      if ((N & 1) == 0 && dispatch_mode() != 2) {  // 2: the load-everything-first five-mode kernel
         const int tiles_per_row = (int)((N + K1T_TILE - 1) / K1T_TILE);
         const long long n_items = (long long)tiles_per_row * B;
         int dev = 0, sms = 148;

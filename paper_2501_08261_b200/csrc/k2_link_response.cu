@@ -22,7 +22,6 @@ constexpr int K2_T = 256;        // output samples per block
 constexpr int K2_THREADS = 128;  // two adjacent samples per thread
 constexpr int K2_G = 16;         // walkers per block (upper bound; 32 measured the same)
 constexpr int K2_NGEO = 21;      // geometry fields per sample
-constexpr bool K2_RMAJOR = true;  // receiver-major sweep order (see the kernel)
 
 struct K2Params {
   int B;
@@ -38,6 +37,7 @@ struct K2Params {
   const double* lambda;
   const double* beta_sky;
   double* y;
+  unsigned int* err;  // sticky device error words (common.cuh)
   OrbitDev orb;
   LagS ls;
 };
@@ -59,12 +59,17 @@ __device__ __forceinline__ void read_pair2(const double2* __restrict__ xe, const
                                            double (&vp)[2], double (&vc)[2]) {
   const double Ka = ceil(Dc[0] + Dla), Kb = ceil(Dc[1] + Dlb);
   const double epsa = (Ka - Dc[0]) - Dla, epsb = (Kb - Dc[1]) - Dlb;
-  // memory safety only (the halo bound keeps every window inside the tile)
-  const int ea = max(elo, min(ea0 - (int)Ka, ehi));
+  // the halo (sized from host-side bounds on the orbit) must keep every window inside the tile;
+  // if it does not, say so (the clamp is for memory safety only: the value is then wrong)
+  int ea = ea0 - (int)Ka, eb = ea0 + 1 - (int)Kb;
+  if (ea < elo || ea > ehi || eb < elo || eb > ehi + 1) {
+    raise_error(p.err, DEVERR_K2_WINDOW);
+    ea = max(elo, min(ea, ehi));
+    eb = max(elo, min(eb, ehi));
+  }
   if (Ka == Kb) {
     lagrange_dot2h_x2<HT>(epsa, epsb, p.half, p.ls, xe, xo, ea, vp, vc);
   } else {
-    const int eb = max(elo, min(ea0 + 1 - (int)Kb, ehi));
     lagrange_dot2h_split(epsa, p.half, p.ls, xe, xo, ea, vp[0], vc[0]);
     lagrange_dot2h_split(epsb, p.half, p.ls, xe, xo, eb, vp[1], vc[1]);
   }
@@ -223,7 +228,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
           Dc[1] = fma(kz, g2.y, Dc[1]);
         }
       }
-      if constexpr (K2_RMAJOR) {
+      {
         // Receiver-major order: iteration k handles spacecraft k as RECEIVER -- its reception-time read
         // and the two links it receives: link +(k+2) from spacecraft k+1 and link -(k+1) from spacecraft
         // k+2 (indices mod 3).  The offsets of the three spacecraft are re-read from geo[] by runtime
@@ -272,64 +277,6 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
           store2(k1 + 3, fma(xpB[0], hps[0] - hpr[0], xcB[0] * (hcs[0] - hcr[0])) * fB[0],
                  fma(xpB[1], hps[1] - hpr[1], xcB[1] * (hcs[1] - hcr[1])) * fB[1]);
         }
-      } else {
-      // per spacecraft slot: k.offset, u.offset, v.offset (samples) and the reception-time
-      // reads h(t - k.r_r/c).  The loops below are NOT unrolled (the unrolled body overflowed
-      // the instruction cache); instead the three slots are rotated after every pass, so the
-      // loop body always addresses the same registers.
-      double kd[3][2], ud[3][2], vd[3][2], hpr[3][2], hcr[3][2];
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        const double2 dx = GEO2(2 + 3 * k), dy = GEO2(3 + 3 * k), dz = GEO2(4 + 3 * k);
-        kd[k][0] = fma(kx, dx.x, fma(ky, dy.x, kz * dz.x));
-        kd[k][1] = fma(kx, dx.y, fma(ky, dy.y, kz * dz.y));
-        ud[k][0] = fma(ux, dx.x, uy * dy.x);
-        ud[k][1] = fma(ux, dx.y, uy * dy.y);
-        vd[k][0] = fma(vx, dx.x, fma(vy, dy.x, vz * dz.x));
-        vd[k][1] = fma(vx, dx.y, fma(vy, dy.y, vz * dz.y));
-        hpr[k][0] = hpr[k][1] = hcr[k][0] = hcr[k][1] = 0.0;
-      }
-#define ROT3(x)                                                  \
-  do {                                                           \
-    const double t0_ = x[0][0], t1_ = x[0][1];                   \
-    x[0][0] = x[1][0]; x[0][1] = x[1][1];                        \
-    x[1][0] = x[2][0]; x[1][1] = x[2][1];                        \
-    x[2][0] = t0_; x[2][1] = t1_;                                \
-  } while (0)
-#pragma unroll 1
-      for (int k = 0; k < 3; ++k) {  // slot 0 holds spacecraft k
-        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, kd[0][0], kd[0][1], p, hpr[0], hcr[0]);
-        ROT3(kd); ROT3(hpr); ROT3(hcr);  // ud, vd are not read here and three rotations are the identity
-      }
-      // three arms; links a and -a share x+, xx and have opposite n.  Arm a joins spacecraft
-      // link_s(a) = a+2 and link_r(a) = a+1 (mod 3): after a rotations they sit in slots 2, 1.
-#pragma unroll 1
-      for (int a = 0; a < 3; ++a) {
-        const double2 Lp = GEO2(11 + a), Lm = GEO2(14 + a), il = GEO2(17 + a);
-        const double ila[2] = {il.x, il.y};
-        double xp[2], xc2[2], fp[2], fm[2];
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-          const double un = (ud[1][c] - ud[2][c]) * ila[c];
-          const double vn = (vd[1][c] - vd[2][c]) * ila[c];
-          const double kn = (kd[1][c] - kd[2][c]) * ila[c];
-          xp[c] = fma(un, un, -vn * vn);
-          xc2[c] = 2.0 * un * vn;
-          const double om = 1.0 - kn, opl = 1.0 + kn;
-          const double inv = 0.5 / (om * opl);  // 1/(2(1-kn)) = (1+kn) inv, 1/(2(1+kn)) = (1-kn) inv
-          fp[c] = opl * inv;
-          fm[c] = om * inv;
-        }
-        double hps[2], hcs[2];
-        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lp.x + kd[2][0], Lp.y + kd[2][1], p, hps, hcs);  // link +a: s -> r
-        store2(a, fma(xp[0], hps[0] - hpr[1][0], xc2[0] * (hcs[0] - hcr[1][0])) * fp[0],
-               fma(xp[1], hps[1] - hpr[1][1], xc2[1] * (hcs[1] - hcr[1][1])) * fp[1]);
-        read_pair2<HT>(xe, xo, elo, ehi, ea0, Dc, Lm.x + kd[1][0], Lm.y + kd[1][1], p, hps, hcs);  // link -a: r -> s
-        store2(a + 3, fma(xp[0], hps[0] - hpr[2][0], xc2[0] * (hcs[0] - hcr[2][0])) * fm[0],
-               fma(xp[1], hps[1] - hpr[2][1], xc2[1] * (hcs[1] - hcr[2][1])) * fm[1]);
-        ROT3(kd); ROT3(ud); ROT3(vd); ROT3(hpr); ROT3(hcr);
-      }
-#undef ROT3
       }
     } else {
 #pragma unroll
@@ -349,13 +296,18 @@ constexpr int K2L_G = 32;
 
 __device__ __forceinline__ void read_pair_lin(const double* __restrict__ hp, const double* __restrict__ hc,
                                               long long na, long long N, const double (&Dc)[2], double Dla,
-                                              double Dlb, double (&vp)[2], double (&vc)[2]) {
+                                              double Dlb, unsigned int* err, double (&vp)[2], double (&vc)[2]) {
   const double Ka = ceil(Dc[0] + Dla), Kb = ceil(Dc[1] + Dlb);
   const double epsa = (Ka - Dc[0]) - Dla, epsb = (Kb - Dc[1]) - Dlb;
-  // taps j = 0, 1: x[n - K], x[n - K + 1] with weights 1 - eps, eps (clamped for memory safety
-  // only: margin_y keeps every window inside [0, N))
-  const long long ia = max(0LL, min(na - (long long)Ka, N - 2));
-  const long long ib = max(0LL, min(na + 1 - (long long)Kb, N - 2));
+  // taps j = 0, 1: x[n - K], x[n - K + 1] with weights 1 - eps, eps.  margin_y (checked on the host
+  // against bounds on the orbit) keeps every window inside [0, N); if it does not, say so (the
+  // clamp is for memory safety only).  The odd-N tail sample na + 1 = N is never stored.
+  long long ia = na - (long long)Ka, ib = na + 1 - (long long)Kb;
+  if (ia < 0 || ia > N - 2 || ib < 0 || ib > N - 1) {
+    raise_error(err, DEVERR_K2_WINDOW);
+    ia = max(0LL, min(ia, N - 2));
+  }
+  ib = max(0LL, min(ib, N - 2));
   const double a0 = __ldg(hp + ia), a1 = __ldg(hp + ia + 1);
   const double c0 = __ldg(hc + ia), c1 = __ldg(hc + ia + 1);
   const bool shared_tap = ib == ia + 1;  // same integer delay: sample b starts on a's second tap
@@ -437,7 +389,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response_lin(const K2Pa
       ud[k][1] = fma(ux, dx.y, uy * dy.y);
       vd[k][0] = fma(vx, dx.x, fma(vy, dy.x, vz * dz.x));
       vd[k][1] = fma(vx, dx.y, fma(vy, dy.y, vz * dz.y));
-      read_pair_lin(hp, hc, na, p.N, Dc, kd[k][0], kd[k][1], hpr[k], hcr[k]);  // h(t - k.r_k/c)
+      read_pair_lin(hp, hc, na, p.N, Dc, kd[k][0], kd[k][1], p.err, hpr[k], hcr[k]);  // h(t - k.r_k/c)
     }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {  // links a and -a share x+, xx and have opposite n
@@ -458,10 +410,10 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response_lin(const K2Pa
         fm[c] = om * inv;
       }
       double hps[2], hcs[2];
-      read_pair_lin(hp, hc, na, p.N, Dc, Lp.x + kd[sd][0], Lp.y + kd[sd][1], hps, hcs);  // link +a: s -> r
+      read_pair_lin(hp, hc, na, p.N, Dc, Lp.x + kd[sd][0], Lp.y + kd[sd][1], p.err, hps, hcs);  // link +a: s -> r
       store2(a, fma(xp[0], hps[0] - hpr[rc][0], xc2[0] * (hcs[0] - hcr[rc][0])) * fp[0],
              fma(xp[1], hps[1] - hpr[rc][1], xc2[1] * (hcs[1] - hcr[rc][1])) * fp[1]);
-      read_pair_lin(hp, hc, na, p.N, Dc, Lm.x + kd[rc][0], Lm.y + kd[rc][1], hps, hcs);  // link -a: r -> s
+      read_pair_lin(hp, hc, na, p.N, Dc, Lm.x + kd[rc][0], Lm.y + kd[rc][1], p.err, hps, hcs);  // link -a: r -> s
       store2(a + 3, fma(xp[0], hps[0] - hpr[sd][0], xc2[0] * (hcs[0] - hcr[sd][0])) * fm[0],
              fma(xp[1], hps[1] - hpr[sd][1], xc2[1] * (hcs[1] - hcr[sd][1])) * fm[1]);
     }
@@ -491,6 +443,7 @@ struct LaserParams {
   long long margin;
   const double* p;
   double* y;
+  unsigned int* err;
   OrbitDev orb;
   LagW lw;
 };
@@ -509,7 +462,10 @@ __global__ void __launch_bounds__(256) k_laser_links(const LaserParams q) {
     const double Kf = ceil(D);
     const double eps = Kf - D;
     long long b = n - (long long)Kf;
-    b = max((long long)(q.half - 1), min(b, q.N - 1 - q.half));
+    if (b < q.half - 1 || b > q.N - 1 - q.half) {  // the margin did not cover the delay after all
+      raise_error(q.err, DEVERR_LASER_WINDOW);
+      b = max((long long)(q.half - 1), min(b, q.N - 1 - q.half));
+    }
     q.y[(size_t)l * q.N + n] = lagrange_dot1<0>(eps, q.half, q.lw, q.p + b) - q.p[n];
   }
 }
@@ -534,7 +490,6 @@ static int launch_k2(const K2Params& p, cudaStream_t st) {
   return LISA_TD_OK;
 }
 
-int g_force_generic = 0;  // debug switch (lisa_td_debug_force_generic)
 
 int run_link_response(int B, long long N, double t0, double dt, int order, long long margin_y,
                       const double* hplus, const double* hcross, const double* lambda,
@@ -545,15 +500,17 @@ int run_link_response(int B, long long N, double t0, double dt, int order, long 
   p.half = (order + 1) / 2; p.margin = (int)margin_y;
   p.hplus = hplus; p.hcross = hcross; p.lambda = lambda; p.beta_sky = beta_sky; p.y = y;
   p.orb = orb;
+  p.err = device_error_words();
   p.group = B < K2_G ? B : K2_G;
   // |K - Kc| <= |Dl| + drift of Dc over the tile + 1.5; the pair window adds half + 1
   p.halo = (int)ceil((orb.max_off_over_c + orb.max_L) / dt + orb.max_dc_rate * K2_T + 1.5) + p.half + 2;
   make_lags(order, &p.ls);
-  if (!g_force_generic && p.half == 1 && !up2) {  // the paper's linear interpolation: its own kernel
+  const bool generic = dispatch_mode() == 1;
+  if (!generic && p.half == 1 && !up2) {  // the paper's linear interpolation: its own kernel
     p.group = B < K2L_G ? B : K2L_G;
     return launch_k2_lin(p, st);
   }
-  if (!g_force_generic) {
+  if (!generic) {
     switch (p.half) {
       case 1: return launch_k2<1>(p, st);
       case 2: return launch_k2<2>(p, st);
@@ -570,7 +527,7 @@ int run_laser_links(long long N, double t0, double dt, int order, long long marg
                     const double* pser, const OrbitDev& orb, double* y, cudaStream_t st) {
   LaserParams q;
   q.N = N; q.t0 = t0; q.dt = dt; q.inv_dt = 1.0 / dt; q.half = (order + 1) / 2;
-  q.margin = margin; q.p = pser; q.y = y; q.orb = orb;
+  q.margin = margin; q.p = pser; q.y = y; q.orb = orb; q.err = device_error_words();
   make_lagw(order, &q.lw);
   k_laser_links<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(q);
   LISA_LAUNCH_CHECK("k_laser_links");

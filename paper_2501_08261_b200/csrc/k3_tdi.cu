@@ -2,16 +2,13 @@
 // (Eq. 2.9-2.11; readings A9, A10 of DESIGN.md).
 //
 // The delays of TDI are sums of light travel times L_l(t_n): they depend on time but NOT on
-// the walker.  The fast kernel therefore gives one block a tile of 32 output samples and ALL
-// walkers: each thread (sample, channel x series) first merges the 4 (generation 2) or 2
-// (generation 1.5) delayed reads that hit its y series into ONE stencil of WIN taps held in
-// registers (the interpolation is linear in y, so  sum_t s_t sum_j c_j(eps_t) y[n-K_t+j]  =
-// sum_i C_i y[n+LOW+i]), then streams the walkers through shared memory (cp.async, double
-// buffered) doing WIN FMAs per walker.  48 coefficient sets per output sample are thus paid
-// once per tile instead of once per walker, and 16x32 taps shrink to 4xWIN.
+// the walker.  The fast kernel (k3_tdi_mma, below) therefore merges the delayed reads of every
+// (channel, y series) pair into one stencil per output sample, shared by all walkers, and
+// applies it as a banded matrix product on the FP64 tensor path.
 //
 // A plain one-thread-per-(walker, sample) kernel covers every other order / cadence.
 #include <cuda.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -40,6 +37,7 @@ struct K3Params {
   LagW lw;
   LagS ls;
   K3Pair pair[12];  // [channel X,Y,Z][slot]
+  unsigned int* err;  // sticky device error words (common.cuh)
   signed char path[3][2][8];  // chained delays: link indices of the two light paths per channel
 };
 
@@ -195,10 +193,9 @@ __device__ __forceinline__ void combine_out(int out_kind, double X, double Y, do
 }
 
 // ---------------------------------------------------------------- generic kernel
-__global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
-  const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const int b = blockIdx.y;
-  if (n >= p.N) return;
+// One (walker, sample): every delayed read its own stencil of runtime (HT = 0) or compile-time order.
+template <int HT>
+__device__ __forceinline__ void k3_generic_sample(const K3Params& p, long long n, int b) {
   double* ob = p.tdi + (size_t)b * 3 * p.N;
   if (n < p.margin_lo || n >= p.N - p.margin_hi) {
     for (int c = 0; c < 3; ++c) ob[(size_t)c * p.N + n] = 0.0;
@@ -225,8 +222,11 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
         const double Kf = ceil(D);
         const double eps = Kf - D;
         long long base = n - (long long)Kf;
-        base = max((long long)(p.half - 1), min(base, p.N - 1 - p.half));
-        acc += (double)pr.t[k].sign * lagrange_dot1<0>(eps, p.half, p.lw, ser + base);
+        if (base < p.half - 1 || base > p.N - 1 - p.half) {  // the margins did not cover the delay after all
+          raise_error(p.err, DEVERR_K3_WINDOW);
+          base = max((long long)(p.half - 1), min(base, p.N - 1 - p.half));
+        }
+        acc += (double)pr.t[k].sign * lagrange_dot1<HT>(eps, p.half, p.lw, ser + base);
       }
     }
     xyz[c] = acc;
@@ -236,31 +236,69 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
   for (int c = 0; c < 3; ++c) ob[(size_t)c * p.N + n] = o[c];
 }
 
+// One thread per (walker, sample): the whole job for orders / cadences the merged-stencil kernel has
+// no instantiation for.
+__global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
+  const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < p.N) k3_generic_sample<0>(p, n, blockIdx.y);
+}
+
+// Fix-up pass behind the merged-stencil kernel: recomputes, sample by sample, the tiles of `tile`
+// samples that k3_anchor_tables listed (list[0] = count, list[1..] = tile indices).  Work item =
+// (listed tile, group of 8 walkers), thread = (sample, walker); blocks without an item leave at once.
+template <int HT>
+__global__ void __launch_bounds__(256) k3_tdi_fixup(const K3Params p, const int* __restrict__ list, const int tile) {
+  const int groups = (p.B + 7) / 8;
+  const int items = list[0] * groups;
+  for (int item = blockIdx.x; item < items; item += gridDim.x) {
+    const long long n = (long long)list[1 + item / groups] * tile + (threadIdx.x % tile);
+    const int b = (item % groups) * 8 + threadIdx.x / tile;
+    if (n < p.N && b < p.B) k3_generic_sample<HT>(p, n, b);
+  }
+}
+
 // ---------------------------------------------------------------- merged-stencil DMMA kernel
-// Block = K3_TS = 32 output samples x ALL walkers.
+// The delays of TDI are sums (or chains) of light travel times: they depend on time but NOT on
+// the walker, and they change by ~1e-7 samples per sample.  The kernel uses both facts.
 //
-// Phase 1 (once per block): warp = (channel, series) pair, lane = sample.  Each thread merges
-// the 4 (generation 2) or 2 (generation 1.5) delayed reads of its pair into ONE stencil of WIN
-// taps (the interpolation is linear in y: sum_t s_t sum_j c_j(eps_t) y[n-K_t+j] = sum_i C_i
-// y[n+LOW+i]) and parks it in shared memory.  The light travel times of the 32 samples are
-// evaluated once (32 threads) and shared.
+// Tile = K3_TS = 32 output samples x ALL walkers.  Per (channel, y series) pair the 4 (generation
+// 2) or 2 (generation 1.5) delayed reads that hit the series merge into ONE stencil of WIN taps
+// (the interpolation is linear in y:  sum_t s_t sum_j c_j(eps_t) y[n-K_t+j] = sum_i C_i y[n+LOW+i]),
+// so the output is a banded product  out[n][w] = sum_pairs sum_m Cband_p[n][m] y_{series(p)}[m][w]
+// whose left operand is shared by every walker: it runs on the FP64 tensor path (mma.sync m8n8k4
+// f64 -> DMMA.8x8x4), warp = (channel, block of 8 samples), A fragments (4 pairs x KSTEPS) in
+// registers for the whole tile, B fragments (y of 8 walkers x 4 times) one conflict-free LDS.64
+// each.  Walkers stream through shared memory in chunks of 16, one 2-D tensor-map TMA copy per
+// chunk (double buffered, mbarrier completion); X,Y,Z of a chunk meet in shared memory for A,E,T.
 //
-// Phase 2: the merged stencils form, per pair, a banded matrix Cband[n][m]; the output is the
-// banded product  out[n][w] = sum_pairs sum_m Cband_p[n][m] y_{series(p)}[m][w]  over the
-// walkers w -- the one dense-ish contraction on this path whose left operand does NOT depend
-// on the walker.  It runs on the FP64 tensor path (mma.sync m8n8k4 f64 -> DMMA.8x8x4): warp =
-// (channel, block of 8 samples), A fragments (4 pairs x KSTEPS) live in registers for the
-// whole block, B fragments (y of 8 walkers x 4 times) are one conflict-free LDS.64 each, and
-// the four pairs of a channel accumulate in the same two accumulator registers.  One LDS.64
-// per 8 FMA instead of one per FMA (the previous SIMT version was shared-memory bound at 22 %
-// FP64-pipe activity).  Walkers stream through shared memory in chunks of 16 (cp.async,
-// double buffered); X,Y,Z of a chunk meet in shared memory for the A,E,T combination.
-constexpr int K3_TS = 32;                  // output samples per block (two 8-row MMA blocks)
-constexpr int K3_PAIRS = 12;               // (channel, series) pairs
-constexpr int K3_THREADS = K3_TS * K3_PAIRS;  // phase 1: thread = (pair, sample); phase 2: warp = (channel, row block)
-constexpr int K3_RB = K3_TS / 8;           // 8-row blocks per tile
-constexpr int K3_WC = 16;                  // walkers per shared-memory chunk (two MMA N-blocks)
-constexpr int K3_XS = K3_WC + 1;           // row stride of the X,Y,Z exchange buffer
+// Merged stencils from three anchors.  Within a tile no integer delay changes (checked), so every
+// tap of the merged stencil is a smooth function of the sample: it is evaluated EXACTLY at the
+// anchor samples 0, 16, 32 of the tile (3 x 48 coefficient sweeps instead of 32 x 48) and every
+// row gets the quadratic through the anchors (truncation |f'''| 16^3 0.064 < 1e-16 of a tap for
+// |dD/dn| < 1e-6).  Tiles where an integer delay does change (one in ~1e4), where
+// the delay is not smooth enough, or that straddle a node of a tabulated orbit are flagged and
+// listed, and recomputed sample by sample by a fix-up pass (k3_tdi_fixup).
+//
+// The anchor stencils do not depend on the walkers either, and a thirteenth warp to prepare them
+// next to the MMA warps does not fit (the A fragments need 104 of the 168 registers a thread can
+// have at three warps per scheduler; four warps per scheduler cap everyone at 128).  They are
+// therefore written by a small kernel of their own (k3_anchor_tables: 12 x 3 x WIN doubles and a
+// split flag per tile, 13 KB) into a workspace, and the persistent MMA kernel (one block per SM,
+// walking over tiles) pulls the table of the NEXT tile into shared memory with one bulk TMA copy
+// while the walkers of the current tile stream through the DMMA loop.
+constexpr int K3_TS = 32;                     // output samples per tile (four 8-row MMA blocks)
+constexpr int K3_PAIRS = 12;                  // (channel, series) pairs
+constexpr int K3_THREADS = K3_TS * K3_PAIRS;  // 384: warp = (channel, row block)
+// a delay is "a parabola over the tile" if its value at sample 8 is within this many samples of the
+// parabola through samples 0, 16, 32: ~10x the rounding noise of a delay of ~12 samples formed from
+// six square roots (4e-15 rms), far below anything that matters for a tap (|dc/deps| ~ 3)
+constexpr double K3_SMOOTH_TOL = 1e-13;
+constexpr int K3_TAB_TILES = 2;               // tiles per block of k3_anchor_tables
+constexpr int K3_TAB_THREADS = 96;
+constexpr int K3_RB = K3_TS / 8;              // 8-row blocks per tile
+constexpr int K3_WC = 16;                     // walkers per shared-memory chunk (two MMA N-blocks)
+constexpr int K3_XS = K3_WC + 1;              // row stride of the X,Y,Z exchange buffer
+constexpr int K3_AH = K3_TS / 2;              // anchor spacing: anchors at tile samples 0, 16, 32
 
 __device__ __forceinline__ void cp_async8_zfill(void* smem, const void* gmem, bool valid) {
   unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -272,8 +310,6 @@ template <int NKEEP>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP));
 }
-// TMA (bulk async copy) of one contiguous run of global memory into shared memory, completion
-// counted in bytes on an mbarrier.  dst, src and bytes must be multiples of 16.
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count) : "memory");
@@ -305,6 +341,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
         : "memory");
   } while (!done);
 }
+// 1-D bulk TMA copy global -> shared (bytes a multiple of 16), completion on an mbarrier
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, unsigned bytes, uint64_t* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(b))
+               : "memory");
+}
 // D(8x8) += A(8x4, row) * B(4x8, col), fp64.  Lane l holds A[l/4][l%4], B[l%4][l/4] and
 // D[l/4][2(l%4) + {0,1}].
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
@@ -313,10 +355,10 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "d"(a), "d"(b));
 }
 
-// Adds sgn * c_j(eps) into the merged stencil at compile-time offset OFF (scaled weights,
-// common.cuh LagS: 7 fp64 ops per node pair + the two accumulations).
-template <int H, int WIN, int OFF>
-__device__ __forceinline__ void add_term_at(double (&C)[WIN], double eps, double sgn, const LagS& ls) {
+// row[j + H - 1] += sgn * c_j(eps), j = -H+1..H, on a shared-memory row owned by the calling
+// thread (scaled weights, common.cuh LagS: 7 fp64 ops per node pair + the two accumulations).
+template <int H>
+__device__ __forceinline__ void add_term_row(double* __restrict__ row, double eps, double sgn, const LagS& ls) {
   double P[H + 1];
   const double q = eps * (eps - 1.0);
   P[1] = ls.g * sgn;
@@ -327,22 +369,11 @@ __device__ __forceinline__ void add_term_at(double (&C)[WIN], double eps, double
   for (int k = H; k >= 1; --k) {
     const double a = P[k] * S;
     const double t = a * eps;
-    C[OFF + k + H - 1] += k == 1 ? t : fma(a, (double)(k - 1), t);
-    C[OFF + H - k] += fma(a, (double)k, -t);
+    row[k + H - 1] += k == 1 ? t : fma(a, (double)(k - 1), t);
+    row[H - k] += fma(a, (double)k, -t);
     if (k > 1) S *= fma(ls.rho[k - 1], q, ls.rc[k - 1]);
   }
 }
-template <int H, int WIN, int OFF>
-struct TermDispatch {
-  static __device__ __forceinline__ void run(double (&C)[WIN], int off, double eps, double sgn, const LagS& ls) {
-    if (off == OFF) add_term_at<H, WIN, OFF>(C, eps, sgn, ls);
-    else TermDispatch<H, WIN, OFF - 1>::run(C, off, eps, sgn, ls);
-  }
-};
-template <int H, int WIN>
-struct TermDispatch<H, WIN, -1> {
-  static __device__ __forceinline__ void run(double (&)[WIN], int, double, double, const LagS&) {}
-};
 
 template <int H, int WIN>
 struct K3Geom {
@@ -350,59 +381,176 @@ struct K3Geom {
   static constexpr int LOW = -(KCAP + H - 1);         // offset of stencil tap 0 relative to n
   static constexpr int KSTEPS = (WIN + 7 + 3) / 4;    // k-steps of one 8-sample row block
   static constexpr int PAD = (LOW % 2 != 0) ? 1 : 0;  // the tile starts at the even sample n0 + LOW - PAD (16-byte aligned rows)
-  static constexpr int TWMIN = K3_TS - 8 + 4 * KSTEPS + PAD;  // y samples a block touches per series
+  static constexpr int TWMIN = K3_TS - 8 + 4 * KSTEPS + PAD;  // y samples a tile touches per series
   static constexpr int TW = TWMIN + ((2 - TWMIN % 4) + 4) % 4;  // == 2 mod 4: walker stride 6 TW == 4 or 12 mod 16
-  static constexpr int CS = ((WIN + 2) / 8) * 8 + 5;  // odd, >= WIN, (CS-1) == 4 mod 8: conflict-free fragment reads
   static constexpr int YBUF = K3_WC * 6 * TW;         // doubles per walker-chunk buffer
-  static constexpr int CBUF = K3_PAIRS * K3_TS * CS;  // doubles of the stencil staging area
-  static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange (phase 1 with chained delays: [32][6][8] + [32][3][6])
-  static_assert(XBUF >= K3_TS * (48 + 18), "chained-delay scratch");
-  // y buffer 0 is private (its first TMA copy overlaps the coefficient phase); the stencil
-  // staging area shares its space with y buffer 1, which is first filled after phase 1
-  static constexpr int UNION_PRIV = YBUF + (YBUF > CBUF ? YBUF : CBUF);
-  static constexpr int UNION_ALIAS = (2 * YBUF > CBUF ? 2 * YBUF : CBUF);
-  // linear interpolation (H = 1): the stencils are short, two blocks share an SM
-  static constexpr int BLOCKS_PER_SM = (K3_TS == 16 || H == 1) ? 2 : 1;
-  static constexpr bool PRIVATE0 = (size_t)(UNION_PRIV + 2 * 3 * K3_TS * K3_XS + K3_TS * 6) * sizeof(double) <= (BLOCKS_PER_SM == 2 ? 112 : 227) * 1024;
-  static constexpr int UNION = PRIVATE0 ? UNION_PRIV : UNION_ALIAS;
-  static constexpr size_t SMEM = (size_t)(UNION + XBUF + K3_TS * 6) * sizeof(double);
+  static constexpr int XBUF = 2 * 3 * K3_TS * K3_XS;  // double buffered X,Y,Z exchange
+  static constexpr int QS = WIN | 1;                  // odd row stride of the anchor stencils: conflict-free sweeps
+  static constexpr int QBUF = K3_PAIRS * 3 * QS;      // one table: [pair][anchor][QS]
+  static constexpr int NA = 4;                        // anchor samples 0, 16, 32 and the check sample 8
+  static constexpr int QFLAG = QS - 1;                // spare slot of row 0: the tile's split flag (0.0 / 1.0)
+  static_assert((QBUF * sizeof(double)) % 16 == 0, "bulk copy size");
+  static constexpr size_t SMEM = (size_t)(2 * YBUF + XBUF + 2 * QBUF) * sizeof(double);
+  // linear interpolation (H = 1): short stencils and few registers, two blocks share an SM if they fit
+  static constexpr int BLOCKS_PER_SM = (H == 1 && SMEM <= 113 * 1024) ? 2 : 1;
 };
+
+__device__ __forceinline__ int k3_anchor_sample(int a) { return a == 3 ? K3_AH / 2 : a * K3_AH; }
+
+// Anchor tables.  Block = K3_TAB_TILES tiles.  Phase A: the delays of every tile at its anchor
+// samples n0, n0 + 16, n0 + 32 and at the check sample n0 + 8.  Phase B: thread = (tile, pair,
+// anchor) sweeps the terms of its pair into one row of WIN taps.  A tile is flagged `split` (the MMA
+// kernel then takes the exact per-row path) if an integer delay differs between its anchors, if
+// the delay is not a parabola in the sample to 1e-13 samples (checked at sample 8, where the cubic
+// term equals the largest interpolation error over the tile), or if it straddles a node of a
+// tabulated orbit.  tab: [n_tiles][12][3][QS], flag in slot QFLAG of row 0; flagged tiles are also
+// appended to `list` (count, then tile indices) for the fix-up pass.
+template <int H, int WIN>
+__global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_constant__ K3Params p, double* __restrict__ tab,
+                                                                   int* __restrict__ list, const int n_tiles) {
+  using G = K3Geom<H, WIN>;
+  constexpr int KCAP = G::KCAP, QS = G::QS, NA = G::NA, T = K3_TAB_TILES;
+  __shared__ double rows[T * G::QBUF];
+  __shared__ double Lanc[T * NA * 6];        // light travel times at the anchors
+  __shared__ double Lq[T * NA * 3 * 6];      // KEPLER1, chained delays: L at t, t - h, t - 2h per anchor
+  __shared__ double taus[T * NA * 6 * 8];    // chained delays per anchor and (channel, path)
+  __shared__ int split[T];
+  const int tid = threadIdx.x;
+  const int tile0 = blockIdx.x * T;
+  for (int i = tid; i < T * G::QBUF; i += K3_TAB_THREADS) rows[i] = 0.0;
+  if (tid < T) {
+    int sp = 0;
+    if (p.orb.kind == 2) {  // a tabulated orbit is a different polynomial on either side of a table node
+      const long long n0 = (long long)(tile0 + tid) * K3_TS;
+      const double reach = p.orb.nested ? 8.0 * p.orb.max_L : 0.0;
+      const double ua = (fma((double)n0, p.dt, p.t0) - reach - p.orb.t_tab0) * p.orb.inv_dt_tab;
+      const double ub = (fma((double)(n0 + K3_TS), p.dt, p.t0) - p.orb.t_tab0) * p.orb.inv_dt_tab;
+      sp = floor(ua) != floor(ub);
+    }
+    split[tid] = sp;
+  }
+  // ---- phase A
+  const double hq = 3.5 * p.orb.max_L;
+  if (p.orb.nested) {
+    if (p.orb.kind == 1) {
+      if (tid < T * NA * 3) {
+        const int tl = tid / (NA * 3), a = (tid / 3) % NA, k = tid % 3;
+        const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+        double L[6];
+        orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0) - (double)k * hq, L);
+#pragma unroll
+        for (int l = 0; l < 6; ++l) Lq[tid * 6 + l] = L[l];
+      }
+      __syncthreads();
+    }
+    if (tid < T * NA * 6) {
+      const int tl = tid / (NA * 6), a = (tid / 6) % NA, cp = tid % 6;  // cp = channel * 2 + path
+      const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+      double tau[8];
+      if (p.orb.kind == 1) chain_delays_quad(Lq + (tl * NA + a) * 18, 1.0 / hq, p.path[cp >> 1][cp & 1], tau);
+      else chain_delays(p.orb, fma((double)n, p.dt, p.t0), p.path[cp >> 1][cp & 1], tau);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) taus[tid * 8 + i] = tau[i];
+    }
+  } else if (tid < T * NA) {
+    const int tl = tid / NA, a = tid % NA;
+    const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+    double L[6];
+    orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
+#pragma unroll
+    for (int l = 0; l < 6; ++l) Lanc[tid * 6 + l] = L[l];
+  }
+  __syncthreads();
+  // ---- phase B
+  if (tid < T * K3_PAIRS * 3) {
+    const int tl = tid / (K3_PAIRS * 3), pi = (tid / 3) % K3_PAIRS, a = tid % 3;
+    const K3Pair& pr = p.pair[pi];
+    double* row = rows + (size_t)tl * G::QBUF + (pi * 3 + a) * QS;
+    auto delay = [&](int k, int an) {
+      if (p.orb.nested) {
+        const int chn = pr.t[k].chain;
+        return taus[((tl * NA + an) * 6 + (pi / 4) * 2 + ((chn >> 3) & 1)) * 8 + (chn & 7)] * p.inv_dt;
+      }
+      double L[6];
+#pragma unroll
+      for (int l = 0; l < 6; ++l) L[l] = Lanc[(tl * NA + an) * 6 + l];
+      return term_delay(pr.t[k], L, p.inv_dt);
+    };
+    for (int k = 0; k < pr.n_terms; ++k) {
+      const double D = delay(k, a);
+      const double Kf = ceil(D);
+      if (a == 0) {
+        const double D1 = delay(k, 1), D2 = delay(k, 2), D8 = delay(k, 3);
+        const bool same_k = Kf == ceil(D1) && Kf == ceil(D2) && Kf == ceil(D8);
+        const bool smooth = fabs(fma(0.375, D, fma(0.75, D1, -0.125 * D2)) - D8) <= K3_SMOOTH_TOL;
+        if (!(same_k && smooth)) split[tl] = 1;
+      }
+      int off = KCAP - (int)Kf;
+      if (off < 0 || off > KCAP) {  // the host-side bound on the delays was wrong
+        raise_error(p.err, DEVERR_K3_WINDOW);
+        off = max(0, min(off, KCAP));
+      }
+      add_term_row<H>(row + off, Kf - D, (double)pr.t[k].sign, p.ls);
+    }
+  }
+  __syncthreads();
+  if (tid < T && tile0 + tid < n_tiles) {
+    rows[(size_t)tid * G::QBUF + G::QFLAG] = split[tid] ? 1.0 : 0.0;
+    if (split[tid]) list[1 + atomicAdd(list, 1)] = tile0 + tid;  // for the fix-up pass (list[0] zeroed by the host)
+  }
+  __syncthreads();
+  const int nt = min(T, n_tiles - tile0);
+  double* dst = tab + (size_t)tile0 * G::QBUF;
+  for (int i = tid; i < nt * G::QBUF; i += K3_TAB_THREADS) dst[i] = rows[i];
+}
 
 template <int H, int WIN>
 __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
-    k3_tdi_mma(const K3Params p, const __grid_constant__ CUtensorMap tmap, const int use_tma) {
+    k3_tdi_mma(const __grid_constant__ K3Params p, const __grid_constant__ CUtensorMap tmap, const int use_tma,
+               const double* __restrict__ tab, const int n_tiles) {
   using G = K3Geom<H, WIN>;
-  constexpr int KCAP = G::KCAP, LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, CS = G::CS, PAD = G::PAD;
+  constexpr int LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, PAD = G::PAD, QS = G::QS;
   constexpr int NWARPS = K3_THREADS / 32;
-  __shared__ __align__(8) uint64_t mbar[2];  // one per walker-chunk buffer (TMA completion)
-  static_assert(CS >= WIN && (CS & 1), "stencil row stride");
+  __shared__ __align__(8) uint64_t ybar[2];    // TMA completion, one per walker-chunk buffer
+  __shared__ __align__(8) uint64_t tbar[2];    // TMA completion, one per anchor-table buffer
   extern __shared__ __align__(128) double smem[];
-  double* ys = smem;                    // [2][WC][6][TW]   (phase 2)
-  double* cbuf = smem + (G::PRIVATE0 ? G::YBUF : 0);  // [12][32][CS]  (phase 1; aliased with y buffer 1, or with both)
-  double* xs = smem + G::UNION;         // [2][3][TS][XS]
-  double* Ls = xs + G::XBUF;            // [32][6]
+  double* ys = smem;                       // [2][WC][6][TW]
+  double* xs = ys + 2 * G::YBUF;           // [2][3][TS][XS]
+  double* qtab = xs + G::XBUF;             // [2][12][3][QS]
   const int lane = threadIdx.x & 31;
   const int wid = threadIdx.x >> 5;
-  const long long n0 = (long long)blockIdx.x * K3_TS;
 
   if (threadIdx.x == 0) {
-    mbar_init(&mbar[0], 1);
-    mbar_init(&mbar[1], 1);
+    mbar_init(&ybar[0], 1);
+    mbar_init(&ybar[1], 1);
+    mbar_init(&tbar[0], 1);
+    mbar_init(&tbar[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
+  __syncthreads();
+  const int my_tiles = ((int)n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  auto tile_id = [&](int it) { return (long long)blockIdx.x + (long long)it * gridDim.x; };
+  auto tile_n0 = [&](int it) { return tile_id(it) * K3_TS; };
+  auto fetch_table = [&](int it) {  // thread 0: anchor table of this block's tile `it` into buffer it & 1
+    mbar_arrive_expect_tx(&tbar[it & 1], (unsigned)(G::QBUF * sizeof(double)));
+    tma_load_1d(qtab + (it & 1) * G::QBUF, tab + (size_t)tile_id(it) * G::QBUF, (unsigned)(G::QBUF * sizeof(double)), &tbar[it & 1]);
+  };
+  if (threadIdx.x == 0 && my_tiles > 0) fetch_table(0);
+
+  // =============================================================== MMA warps
   const int n_chunks = (p.B + K3_WC - 1) / K3_WC;
   // Walker chunks arrive by TMA: ONE 2-D tiled copy per chunk (box = TW samples x 96 rows of the
   // [B*6][N] matrix; parts of the box outside the matrix are zero-filled by the hardware, which
   // covers both the grid edges and a ragged last chunk), completion counted on the buffer's
   // mbarrier.  The tensor map needs 16-byte row strides, so odd N takes the zero-filling
   // cp.async path instead.
-  const long long g0 = n0 + LOW - PAD;
-  auto prefetch = [&](int chunk, int buf) {
+  auto prefetch = [&](long long n0, int chunk, int buf) {
     double* dst = ys + (size_t)buf * G::YBUF;
+    const long long g0 = n0 + LOW - PAD;
     if (use_tma) {
       if (threadIdx.x == 0) {
-        mbar_arrive_expect_tx(&mbar[buf], (unsigned)(G::YBUF * sizeof(double)));
-        tma_load_2d(dst, &tmap, (int)g0, chunk * K3_WC * 6, &mbar[buf]);
+        mbar_arrive_expect_tx(&ybar[buf], (unsigned)(G::YBUF * sizeof(double)));
+        tma_load_2d(dst, &tmap, (int)g0, chunk * K3_WC * 6, &ybar[buf]);
       }
     } else {
       const int nrows = min(K3_WC, p.B - chunk * K3_WC) * 6;
@@ -418,150 +566,108 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
       cp_async_commit();
     }
   };
-  if (G::PRIVATE0) prefetch(0, 0);  // chunk 0 lands in y buffer 0 while the coefficients are computed
-  // ---- phase 1a: light travel times of the tile's samples
-  // (chained delays, A22: thread = (sample, channel, light path) walks its path leg by leg and
-  // parks the 8 delays in the X,Y,Z exchange area, which phase 2 has not touched yet)
-  double* taus = xs;  // [32][3][2][8]
-  if (p.orb.nested) {
-    double* Lq = taus + K3_TS * 6 * 8;  // [32][3][6]: KEPLER1 only
-    const double hq = 3.5 * p.orb.max_L;
-    if (p.orb.kind == 1) {
-      if (threadIdx.x < K3_TS * 3) {
-        const int sm = threadIdx.x % K3_TS, k = threadIdx.x / K3_TS;
-        double L[6];
-        orbit_arm_times(p.orb, fma((double)(n0 + sm), p.dt, p.t0) - (double)k * hq, L);
-#pragma unroll
-        for (int l = 0; l < 6; ++l) Lq[(sm * 3 + k) * 6 + l] = L[l];
-      }
-      __syncthreads();
-    }
-    if (threadIdx.x < K3_TS * 6) {
-      const int sm = threadIdx.x % K3_TS, cp = threadIdx.x / K3_TS;  // cp = channel * 2 + path
-      double tau[8];
-      if (p.orb.kind == 1) chain_delays_quad(Lq + sm * 18, 1.0 / hq, p.path[cp >> 1][cp & 1], tau);
-      else chain_delays(p.orb, fma((double)(n0 + sm), p.dt, p.t0), p.path[cp >> 1][cp & 1], tau);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) taus[(sm * 6 + cp) * 8 + i] = tau[i];
-    }
-  } else if (threadIdx.x < K3_TS) {
-    double L[6];
-    orbit_arm_times(p.orb, fma((double)(n0 + threadIdx.x), p.dt, p.t0), L);
-#pragma unroll
-    for (int l = 0; l < 6; ++l) Ls[threadIdx.x * 6 + l] = L[l];
-  }
-  __syncthreads();
-  // ---- phase 1b: merged stencil of (pair = wid, sample = lane)
-  {
-    double C[WIN];
-#pragma unroll
-    for (int i = 0; i < WIN; ++i) C[i] = 0.0;
-    const int pi = threadIdx.x / K3_TS, sm = threadIdx.x % K3_TS;  // pair, sample
-    const K3Pair& pr = p.pair[pi];
-    const long long n = n0 + sm;
-    if (n >= p.margin_lo && n < p.N - p.margin_hi) {
-      double L[6];
-#pragma unroll
-      for (int l = 0; l < 6; ++l) L[l] = Ls[sm * 6 + l];
-      for (int k = 0; k < pr.n_terms; ++k) {
-        const int chn = pr.t[k].chain;
-        const double D = p.orb.nested ? taus[(sm * 6 + (pi / 4) * 2 + ((chn >> 3) & 1)) * 8 + (chn & 7)] * p.inv_dt
-                                      : term_delay(pr.t[k], L, p.inv_dt);
-        const double Kf = ceil(D);
-        const double eps = Kf - D;
-        int off = KCAP - (int)Kf;
-        off = max(0, min(off, KCAP));
-        TermDispatch<H, WIN, KCAP>::run(C, off, eps, (double)pr.t[k].sign, p.ls);
-      }
-    }
-    double* dst = cbuf + (size_t)(pi * K3_TS + sm) * CS;
-#pragma unroll
-    for (int i = 0; i < WIN; ++i) dst[i] = C[i];
-  }
-  __syncthreads();
-  // ---- phase 1c: A fragments of (channel ch, row block rb): 4 pairs x KSTEPS values
   const int ch = wid / K3_RB, rb = wid % K3_RB;
   const int r = lane >> 2, kk = lane & 3;
-  double A[4][KSTEPS];
   int ser[4];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    ser[q] = p.pair[ch * 4 + q].series;
-    const double* src = cbuf + (size_t)((ch * 4 + q) * K3_TS + rb * 8 + r) * CS;
-#pragma unroll
-    for (int ks = 0; ks < KSTEPS; ++ks) {
-      const int i = 4 * ks + kk - r;
-      A[q][ks] = (i >= 0 && i < WIN) ? src[i] : 0.0;
-    }
-  }
-  // cbuf (generic-proxy writes and reads) is about to become y buffer 1 (async-proxy TMA writes):
-  // every thread that touched it fences, THEN the barrier, then one thread issues the copy
-  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-  __syncthreads();  // cbuf is dead from here on: its space becomes the y buffers
+  for (int q = 0; q < 4; ++q) ser[q] = p.pair[ch * 4 + q].series;
+  const bool vec = (p.N & 1) == 0;
 
-  // ---- phase 2: stream walkers
-  if (!G::PRIVATE0) prefetch(0, 0);
-  for (int c = 0; c < n_chunks; ++c) {
-    const int buf = c & 1;
-    if (c + 1 < n_chunks) prefetch(c + 1, buf ^ 1);
-    if (use_tma) {
-      mbar_wait(&mbar[buf], (unsigned)((c >> 1) & 1));
-    } else {
-      if (c + 1 < n_chunks) cp_async_wait<1>();
-      else cp_async_wait<0>();
-    }
-    // TMA path: the mbarrier wait makes the tile visible to each waiting thread, and the
-    // X,Y,Z exchange buffer alternates, so ONE barrier per chunk (after the MMAs) is enough:
-    // warps that finish their stores early start the next chunk's MMAs.
-    if (!use_tma) __syncthreads();  // cp.async path: other threads' copies become visible here
-    double* xsc = xs + (size_t)buf * (3 * K3_TS * K3_XS);
-    // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
-    const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
-    double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const double* y0 = yb + ser[q] * TW;
-      const double* y1 = y0 + 8 * 6 * TW;
-#pragma unroll
-      for (int ks = 0; ks < KSTEPS; ++ks) {
-        dmma884(d00, d01, A[q][ks], y0[4 * ks]);
-        dmma884(d10, d11, A[q][ks], y1[4 * ks]);
-      }
-    }
+  if (my_tiles > 0) prefetch(tile_n0(0), 0, 0);
+  unsigned g = 0;  // chunks processed so far (y and exchange buffers alternate on it)
+  for (int it = 0; it < my_tiles; ++it) {
+    const int tb = it & 1;
+    const long long n0 = tile_n0(it);
+    // the table buffer of the next tile was last read by the A fragments of the previous tile,
+    // which every warp completed before the barriers of that tile's chunks
+    if (threadIdx.x == 0 && it + 1 < my_tiles) fetch_table(it + 1);
+    mbar_wait(&tbar[tb], (unsigned)((it >> 1) & 1));
+    // ---- A fragments of (channel ch, row block rb): 4 pairs x KSTEPS values
+    const double* qt = qtab + tb * G::QBUF;
+    // (a tile whose table carries the split flag gets meaningless fragments here: the fix-up pass
+    // behind this kernel overwrites its outputs)
+    double A[4][KSTEPS];
     {
-      double* xr = xsc + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
-      xr[0] = d00; xr[1] = d01; xr[8] = d10; xr[9] = d11;
-    }
-    __syncthreads();  // X,Y,Z of chunk c complete; every warp is done reading y buffer `buf`
-    // thread = (walker, two adjacent samples): X,Y,Z -> the three output channels, one 16-byte
-    // store per channel
-    const bool vec = (p.N & 1) == 0;
-    for (int e = threadIdx.x; e < K3_WC * (K3_TS / 2); e += K3_THREADS) {
-      const int l2 = e % (K3_TS / 2), w = e / (K3_TS / 2);
-      const int b = c * K3_WC + w;
-      const long long nn = n0 + 2 * l2;
-      if (b >= p.B || nn >= p.N) continue;
-      double v[3][2];
+      // weights of the three anchors at this lane's row (quadratic through samples 0, 16, 32)
+      const double u = (double)(rb * 8 + r) * (1.0 / K3_AH);
+      const double w0 = 0.5 * (u - 1.0) * (u - 2.0), w1 = u * (2.0 - u), w2 = 0.5 * u * (u - 1.0);
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int ln = 2 * l2 + h;
-        const double X = xsc[(0 * K3_TS + ln) * K3_XS + w];
-        const double Y = xsc[(1 * K3_TS + ln) * K3_XS + w];
-        const double Z = xsc[(2 * K3_TS + ln) * K3_XS + w];
-        double out[3];
-        combine_out(p.out_kind, X, Y, Z, out);
-        const bool zero = nn + h < p.margin_lo || nn + h >= p.N - p.margin_hi;
+      for (int q = 0; q < 4; ++q) {
+        const double* src = qt + (ch * 4 + q) * 3 * QS;
 #pragma unroll
-        for (int o = 0; o < 3; ++o) v[o][h] = zero ? 0.0 : out[o];
+        for (int ks = 0; ks < KSTEPS; ++ks) {
+          const int i = 4 * ks + kk - r;
+          const bool in = i >= 0 && i < WIN;
+          const int ic = in ? i : 0;
+          const double v = fma(w2, src[2 * QS + ic], fma(w1, src[QS + ic], w0 * src[ic]));
+          A[q][ks] = in ? v : 0.0;
+        }
       }
+    }
+
+    // ---- stream the walkers
+    for (int c = 0; c < n_chunks; ++c, ++g) {
+      const int buf = g & 1;
+      // the other y buffer was last read in the previous chunk, which every MMA warp has left
+      bool more = true;
+      if (c + 1 < n_chunks) prefetch(n0, c + 1, buf ^ 1);
+      else if (it + 1 < my_tiles) prefetch(tile_n0(it + 1), 0, buf ^ 1);
+      else more = false;
+      if (use_tma) {
+        mbar_wait(&ybar[buf], (g >> 1) & 1);
+      } else {
+        if (more) cp_async_wait<1>();
+        else cp_async_wait<0>();
+        __syncthreads();  // cp.async path: other threads' copies become visible here
+      }
+      double* xsc = xs + (size_t)buf * (3 * K3_TS * K3_XS);
+      // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
+      const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
+      double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
 #pragma unroll
-      for (int o = 0; o < 3; ++o) {
-        double* dst = p.tdi + ((size_t)b * 3 + o) * p.N + nn;
-        if (vec) {
-          *reinterpret_cast<double2*>(dst) = make_double2(v[o][0], v[o][1]);
-        } else {
-          dst[0] = v[o][0];
-          if (nn + 1 < p.N) dst[1] = v[o][1];
+      for (int q = 0; q < 4; ++q) {
+        const double* y0 = yb + ser[q] * TW;
+        const double* y1 = y0 + 8 * 6 * TW;
+#pragma unroll
+        for (int ks = 0; ks < KSTEPS; ++ks) {
+          dmma884(d00, d01, A[q][ks], y0[4 * ks]);
+          dmma884(d10, d11, A[q][ks], y1[4 * ks]);
+        }
+      }
+      {
+        double* xr = xsc + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
+        xr[0] = d00; xr[1] = d01; xr[8] = d10; xr[9] = d11;
+      }
+      __syncthreads();  // X,Y,Z of this chunk complete; every warp is done reading y buffer `buf`
+      // thread = (walker, two adjacent samples): X,Y,Z -> the three output channels, one 16-byte
+      // store per channel
+      for (int e = threadIdx.x; e < K3_WC * (K3_TS / 2); e += K3_THREADS) {
+        const int l2 = e % (K3_TS / 2), w = e / (K3_TS / 2);
+        const int b = c * K3_WC + w;
+        const long long nn = n0 + 2 * l2;
+        if (b >= p.B || nn >= p.N) continue;
+        double v[3][2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int ln = 2 * l2 + h;
+          const double X = xsc[(0 * K3_TS + ln) * K3_XS + w];
+          const double Y = xsc[(1 * K3_TS + ln) * K3_XS + w];
+          const double Z = xsc[(2 * K3_TS + ln) * K3_XS + w];
+          double out[3];
+          combine_out(p.out_kind, X, Y, Z, out);
+          const bool zero = nn + h < p.margin_lo || nn + h >= p.N - p.margin_hi;
+#pragma unroll
+          for (int o = 0; o < 3; ++o) v[o][h] = zero ? 0.0 : out[o];
+        }
+#pragma unroll
+        for (int o = 0; o < 3; ++o) {
+          double* dst = p.tdi + ((size_t)b * 3 + o) * p.N + nn;
+          if (vec) {
+            *reinterpret_cast<double2*>(dst) = make_double2(v[o][0], v[o][1]);
+          } else {
+            dst[0] = v[o][0];
+            if (nn + 1 < p.N) dst[1] = v[o][1];
+          }
         }
       }
     }
@@ -583,16 +689,27 @@ static EncodeTiledFn encode_tiled_fn() {
   return fn;
 }
 
+// bytes of workspace run_tdi needs for N samples: the anchor tables (sized for the widest window),
+// then the list of flagged tiles
+static long long tdi_table_bytes(long long n_tiles) {
+  return ((n_tiles * (long long)K3Geom<16, 48>::QBUF * (long long)sizeof(double)) + 255) / 256 * 256;
+}
+long long tdi_workspace_bytes(long long N) {
+  const long long n_tiles = (N + K3_TS - 1) / K3_TS;
+  return tdi_table_bytes(n_tiles) + ((n_tiles + 1) * (long long)sizeof(int) + 255) / 256 * 256;
+}
+
 template <int H, int WIN>
-static int launch_mma(const K3Params& p, cudaStream_t st) {
+static int launch_mma(const K3Params& p, double* tab, cudaStream_t st) {
   using G = K3Geom<H, WIN>;
-  static_assert(G::SMEM <= 227 * 1024, "k3_tdi_mma shared memory");
+  static_assert(G::SMEM <= (G::BLOCKS_PER_SM == 2 ? 113 : 227) * 1024, "k3_tdi_mma shared memory");
   static_assert((G::YBUF * sizeof(double)) % 128 == 0, "TMA destination alignment");
+  static_assert(G::QBUF <= K3Geom<16, 48>::QBUF, "workspace size");
   CUtensorMap tmap;
   memset(&tmap, 0, sizeof(tmap));
   int use_tma = 0;
   EncodeTiledFn enc = encode_tiled_fn();
-  if (enc && (p.N & 1) == 0 && p.N < (1LL << 31)) {
+  if (enc && (p.N & 1) == 0 && p.N < (1LL << 31) - 4096) {
     const cuuint64_t gdim[2] = {(cuuint64_t)p.N, (cuuint64_t)p.B * 6};
     const cuuint64_t gstr[1] = {(cuuint64_t)p.N * sizeof(double)};
     const cuuint32_t box[2] = {(cuuint32_t)G::TW, (cuuint32_t)(K3_WC * 6)};
@@ -602,21 +719,61 @@ static int launch_mma(const K3Params& p, cudaStream_t st) {
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     use_tma = r == CUDA_SUCCESS;
   }
+  const long long n_tiles = (p.N + K3_TS - 1) / K3_TS;
+  // 1. anchor stencils of every tile (walker-independent)
+  int* list = reinterpret_cast<int*>(reinterpret_cast<char*>(tab) + tdi_table_bytes(n_tiles));
+  LISA_CUDA(cudaMemsetAsync(list, 0, sizeof(int), st));
+  k3_anchor_tables<H, WIN><<<(unsigned)((n_tiles + K3_TAB_TILES - 1) / K3_TAB_TILES), K3_TAB_THREADS, 0, st>>>(p, tab, list, (int)n_tiles);
+  LISA_LAUNCH_CHECK("k3_anchor_tables");
+  // 2. persistent MMA blocks: one (two at order 1) per SM, each walking over tiles blockIdx.x + i gridDim.x
   LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-  k3_tdi_mma<H, WIN><<<(unsigned)((p.N + K3_TS - 1) / K3_TS), K3_THREADS, G::SMEM, st>>>(p, tmap, use_tma);
+  const long long resident = (long long)G::BLOCKS_PER_SM * sm_count();
+  const unsigned grid = (unsigned)(n_tiles < resident ? n_tiles : resident);
+  k3_tdi_mma<H, WIN><<<grid, K3_THREADS, G::SMEM, st>>>(p, tmap, use_tma, tab, (int)n_tiles);
   LISA_LAUNCH_CHECK("k3_tdi_mma");
+  // 3. fix-up: the flagged tiles, sample by sample (threads of other tiles leave at once)
+  k3_tdi_fixup<H><<<2 * sm_count(), 256, 0, st>>>(p, list, K3_TS);
+  LISA_LAUNCH_CHECK("k3_tdi_fixup");
   return LISA_TD_OK;
 }
 
-extern int g_force_generic;
+// the merged-stencil path with its workspace: the caller's, or a stream-ordered temporary
+template <int H, int WIN>
+static int run_mma(const K3Params& p, double* tab_ws, long long tab_ws_bytes, cudaStream_t st) {
+  const long long need = tdi_workspace_bytes(p.N);
+  if (tab_ws) {
+    if (tab_ws_bytes < need) return set_error(LISA_TD_ENOMEM, "tdi: workspace of %lld bytes is smaller than the %lld needed", tab_ws_bytes, need);
+    return launch_mma<H, WIN>(p, tab_ws, st);
+  }
+  // no workspace argument (lisa_td_tdi2): draw it from the device's stream-ordered memory pool and
+  // give it back in stream order -- no synchronisation, and the pool keeps the pages for the next call
+  static thread_local int pool_dev = -1;
+  int dev = 0;
+  LISA_CUDA(cudaGetDevice(&dev));
+  if (dev != pool_dev) {
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      unsigned long long keep = ~0ULL;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    cudaGetLastError();
+    pool_dev = dev;
+  }
+  void* tmp = nullptr;
+  LISA_CUDA(cudaMallocAsync(&tmp, (size_t)need, st));
+  const int rc = launch_mma<H, WIN>(p, static_cast<double*>(tmp), st);
+  const int rc2 = check_cuda(cudaFreeAsync(tmp, st), "cudaFreeAsync");
+  return rc ? rc : rc2;
+}
 
 int run_tdi(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
             long long margin_lo, long long margin_hi, const double* y, const OrbitDev& orb,
-            double* tdi, cudaStream_t st) {
+            double* tdi, cudaStream_t st, double* tab_ws, long long tab_ws_bytes) {
   K3Params p;
   p.B = B; p.N = N; p.t0 = t0; p.dt = dt; p.inv_dt = 1.0 / dt;
   p.half = (order + 1) / 2; p.generation = generation; p.out_kind = out_kind;
   p.margin_lo = margin_lo; p.margin_hi = margin_hi; p.y = y; p.tdi = tdi; p.orb = orb;
+  p.err = device_error_words();
   make_lagw(order, &p.lw);
   make_lags(order, &p.ls);
   if (build_pairs(generation, p.pair, p.path))
@@ -625,14 +782,14 @@ int run_tdi(int B, long long N, double t0, double dt, int order, int generation,
   const int kcap = (int)ceil(nL * orb.max_L / dt);
   p.kcap = kcap;
   const int need = kcap + 2 * p.half;
-  if (!g_force_generic) {
+  if (dispatch_mode() != 1) {
     if (p.half == 16) {
-      if (need <= 40) return launch_mma<16, 40>(p, st);
-      if (need <= 44) return launch_mma<16, 44>(p, st);
-      if (need <= 48) return launch_mma<16, 48>(p, st);
+      if (need <= 40) return run_mma<16, 40>(p, tab_ws, tab_ws_bytes, st);
+      if (need <= 44) return run_mma<16, 44>(p, tab_ws, tab_ws_bytes, st);
+      if (need <= 48) return run_mma<16, 48>(p, tab_ws, tab_ws_bytes, st);
     } else if (p.half == 1) {
-      if (need <= 8) return launch_mma<1, 8>(p, st);
-      if (need <= 16) return launch_mma<1, 16>(p, st);
+      if (need <= 8) return run_mma<1, 8>(p, tab_ws, tab_ws_bytes, st);
+      if (need <= 16) return run_mma<1, 16>(p, tab_ws, tab_ws_bytes, st);
     }
   }
   dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);

@@ -25,6 +25,7 @@ namespace lisa {
 
 constexpr int K5_SLICES = 32;
 constexpr int K5_THREADS = 256;
+constexpr int K5_MAX_PLANS = 8;  // cached cuFFT plans per lisa_td_plan (batch sizes a sampler alternates between)
 constexpr int K6_MAXD = 32;     // parameters of the Fisher matrix
 constexpr int K6_TILE = 128;    // (channel, bin) items staged per pass
 constexpr int K6_THREADS = 256;
@@ -33,7 +34,11 @@ constexpr int K6_BLOCKS = 296;  // 2 per SM
 struct Plan {
   int B;  // capacity (walkers)
   long long N, nf;
-  std::map<int, cufftHandle> fft;  // batched D2Z plans keyed by the number of walkers
+  // batched half-length Z2Z plans keyed by (walkers, all channels | one channel); at most
+  // K5_MAX_PLANS of them, all sharing ONE work area (cuFFT's own allocation is switched off)
+  std::map<int, cufftHandle> fft;
+  void* work;
+  size_t work_bytes;
   double2* spec;     // [B][3][M] packed half-length spectra Z (M = N/2)
   double2* partial;  // [B][K5_SLICES]
   double* fisher_partial;  // [K6_BLOCKS][K6_MAXD * K6_MAXD], allocated on first use
@@ -218,11 +223,39 @@ static int get_fft(Plan* pl, int B, cufftHandle* h, int single = 0) {
   size_t ws = 0;
   long long embed[1] = {pl->N / 2};
   const long long dist = single ? 3 * (pl->N / 2) : pl->N / 2;
-  rc = check_fft(cufftMakePlanMany64(f, 1, n, embed, 1, dist, embed, 1, dist, CUFFT_Z2Z, single ? (long long)B : 3LL * B, &ws),
-                 "cufftMakePlanMany64");
+  rc = check_fft(cufftSetAutoAllocation(f, 0), "cufftSetAutoAllocation");
+  if (rc == LISA_TD_OK)
+    rc = check_fft(cufftMakePlanMany64(f, 1, n, embed, 1, dist, embed, 1, dist, CUFFT_Z2Z, single ? (long long)B : 3LL * B, &ws),
+                   "cufftMakePlanMany64");
+  if (rc == LISA_TD_OK && ws > pl->work_bytes) {
+    // a larger work area than any plan so far needed (normally only the capacity plan made in
+    // lisa_td_plan_create gets here): wait for work that may still use the old one, then replace it
+    rc = check_cuda(cudaDeviceSynchronize(), "cudaDeviceSynchronize");
+    void* nw = nullptr;
+    if (rc == LISA_TD_OK) rc = check_cuda(cudaMalloc(&nw, ws), "cudaMalloc(cuFFT work area)");
+    if (rc == LISA_TD_OK) {
+      cudaFree(pl->work);
+      pl->work = nw;
+      pl->work_bytes = ws;
+      for (auto& kv : pl->fft)
+        if (rc == LISA_TD_OK) rc = check_fft(cufftSetWorkArea(kv.second, pl->work), "cufftSetWorkArea");
+    }
+  }
+  if (rc == LISA_TD_OK && ws > 0) rc = check_fft(cufftSetWorkArea(f, pl->work), "cufftSetWorkArea");
   if (rc != LISA_TD_OK) {
     cufftDestroy(f);
     return rc;
+  }
+  if ((int)pl->fft.size() >= K5_MAX_PLANS) {
+    // bounded cache: drop every plan but the capacity plan (key 2 * pl->B); they are re-made on demand
+    for (auto it2 = pl->fft.begin(); it2 != pl->fft.end();) {
+      if (it2->first != 2 * pl->B) {
+        cufftDestroy(it2->second);
+        it2 = pl->fft.erase(it2);
+      } else {
+        ++it2;
+      }
+    }
   }
   pl->fft[key] = f;
   *h = f;
@@ -234,6 +267,7 @@ int plan_destroy(Plan* pl);
 int plan_create(Plan** out, int B, long long N) {
   Plan* pl = new Plan();
   pl->B = B; pl->N = N; pl->nf = N / 2 + 1; pl->spec = nullptr; pl->partial = nullptr; pl->fisher_partial = nullptr;
+  pl->work = nullptr; pl->work_bytes = 0;
   int rc = check_cuda(cudaMalloc(&pl->spec, sizeof(double2) * (size_t)B * 3 * pl->nf), "cudaMalloc(spec)");
   if (rc == LISA_TD_OK) rc = check_cuda(cudaMalloc(&pl->partial, sizeof(double2) * (size_t)B * K5_SLICES), "cudaMalloc(partial)");
   cufftHandle h;
@@ -252,12 +286,15 @@ int plan_destroy(Plan* pl) {
   cudaFree(pl->spec);
   cudaFree(pl->partial);
   cudaFree(pl->fisher_partial);
+  cudaFree(pl->work);
   delete pl;
   return LISA_TD_OK;
 }
 
 // FFT of B <= capacity walkers.  A plan for a batch size not seen before is created on first
-// use (that call synchronises inside cuFFT).
+// use (host work inside cuFFT; no device allocation unless it needs a larger work area than the
+// capacity plan).  The cuFFT handles carry the stream of the last call: a lisa_td_plan must not
+// be used from two host threads at once.
 static int run_fft(Plan* pl, int B, const double* tdi, double2* spec, cudaStream_t st, int n_ch = 3) {
   if (B > pl->B) return set_error(LISA_TD_EINVAL, "B=%d exceeds the plan's capacity %d", B, pl->B);
   cufftHandle h;
@@ -282,18 +319,18 @@ static int run_fft(Plan* pl, int B, const double* tdi, double2* spec, cudaStream
 __global__ void k5_unpack_spectrum(const double2* __restrict__ Z, long long rows, long long nf, double two_pi_over_N,
                                    double2* __restrict__ out) {
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long row = blockIdx.y;
   if (k >= nf) return;
   double cw, sw;
   bin_twiddle(k, two_pi_over_N, cw, sw);
-  out[(size_t)row * nf + k] = packed_bin(Z + (size_t)row * (nf - 1), nf - 1, k, cw, sw);
+  for (long long row = blockIdx.y; row < rows; row += gridDim.y)  // grid.y is capped at 65535
+    out[(size_t)row * nf + k] = packed_bin(Z + (size_t)row * (nf - 1), nf - 1, k, cw, sw);
 }
 
 int run_spectrum(Plan* pl, int B, long long N, const double* tdi, double* spec, cudaStream_t st) {
   if (N != pl->N) return set_error(LISA_TD_EINVAL, "spectrum: N differs from the plan's");
   int rc = run_fft(pl, B, tdi, pl->spec, st);
   if (rc != LISA_TD_OK) return rc;
-  dim3 grid((unsigned)((pl->nf + 255) / 256), (unsigned)(3 * B));
+  dim3 grid((unsigned)((pl->nf + 255) / 256), (unsigned)(3 * B < 65535 ? 3 * B : 65535));
   k5_unpack_spectrum<<<grid, 256, 0, st>>>(pl->spec, 3LL * B, pl->nf, 6.283185307179586476925 / (double)N,
                                            reinterpret_cast<double2*>(spec));
   LISA_LAUNCH_CHECK("k5_unpack_spectrum");

@@ -24,9 +24,9 @@ EXPORTS = [
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
     "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
-    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_pipeline_host_up2", "lisa_td_probe_dfma", "lisa_td_probe_fp64_pipes",
-    "lisa_td_debug_force_generic",
+    "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_pipeline_host_up2", "lisa_td_check",
 ]
+PROBE_LIB_PATH = os.path.join(_HERE, "liblisa_td_probe.so")  # bench-only, csrc/lisa_td_probe.h
 
 
 class LisaTdError(RuntimeError):
@@ -132,10 +132,7 @@ def load() -> C.CDLL:
                                         + [dbl, dbl, i32, i64, i32, i64, i64, C.POINTER(Orbit), vp, vp,
                                            i64, i64, vp, vp, vp])
     L.lisa_td_pipeline_host_up2.argtypes = L.lisa_td_pipeline_host.argtypes
-    L.lisa_td_probe_dfma.argtypes = [i64, i32, i32, vp, C.POINTER(C.c_float), vp]
-    L.lisa_td_probe_fp64_pipes.argtypes = [i64, i32, i32, i32, vp, C.POINTER(C.c_float), vp]
-    L.lisa_td_debug_force_generic.argtypes = [i32]
-    L.lisa_td_debug_force_generic.restype = None
+    L.lisa_td_check.argtypes = [vp]
     _lib = L
     return L
 
@@ -184,8 +181,17 @@ def version() -> int:
     return load().lisa_td_version()
 
 
-def debug_force_generic(on: bool):
-    load().lisa_td_debug_force_generic(int(on))
+def check():
+    """lisa_td_check on the current torch stream: synchronises, raises if a kernel flagged a delay
+    outside the host-side orbit bounds."""
+    _check(load().lisa_td_check(_stream()))
+
+
+def debug_force_generic(mode):
+    """TEST-ONLY dispatch switch (not an ABI call): sets the environment variable LISA_TD_DISPATCH,
+    which the library reads at every call.  1 = generic kernels, 2 = five-mode S1 without TMA,
+    0 / False = normal."""
+    os.environ["LISA_TD_DISPATCH"] = str(int(mode))
 
 
 def modes_to_pol(B, N, l, m, amp, phase, alpha, beta, gamma, iota, phi, psi, euler0, hplus, hcross):
@@ -319,13 +325,32 @@ def pipeline_host_up2(pipe: Pipeline, B, N, l, m, amp_c, phase_c, alpha_c, beta_
         kmax, _host(loglike_out), _host(dh), _host(hh)))
 
 
+_probe = None
+
+
+def _probe_lib() -> C.CDLL:
+    """liblisa_td_probe.so: fp64 throughput probes for bench.py (csrc/lisa_td_probe.h), not product ABI"""
+    global _probe
+    if _probe is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            raise ImportError(f"{PROBE_LIB_PATH} not built; run `python -m paper_2501_08261_b200.build`")
+        P = C.CDLL(PROBE_LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int, C.c_longlong
+        P.lisa_td_probe_dfma.argtypes = [i64, i32, i32, vp, C.POINTER(C.c_float), vp]
+        P.lisa_td_probe_fp64_pipes.argtypes = [i64, i32, i32, i32, vp, C.POINTER(C.c_float), vp]
+        _probe = P
+    return _probe
+
+
 def probe_dfma(iters, blocks, threads, sink) -> float:
     ms = C.c_float()
-    _check(load().lisa_td_probe_dfma(iters, blocks, threads, _dev(sink), C.byref(ms), _stream()))
+    if _probe_lib().lisa_td_probe_dfma(iters, blocks, threads, _dev(sink), C.byref(ms), _stream()) != 0:
+        raise RuntimeError("lisa_td_probe_dfma failed")
     return ms.value
 
 
 def probe_fp64_pipes(iters, blocks, dfma_warps, dmma_warps, sink) -> float:
     ms = C.c_float()
-    _check(load().lisa_td_probe_fp64_pipes(iters, blocks, dfma_warps, dmma_warps, _dev(sink), C.byref(ms), _stream()))
+    if _probe_lib().lisa_td_probe_fp64_pipes(iters, blocks, dfma_warps, dmma_warps, _dev(sink), C.byref(ms), _stream()) != 0:
+        raise RuntimeError("lisa_td_probe_fp64_pipes failed")
     return ms.value

@@ -267,7 +267,7 @@ def _gpu_chain(lib, inp, gen=20, out_kind=1, want_y=False):
     lib.response_tdi(B, N, inp["t0"], inp["dt"], inp["order"], inp["margin_y"], gen, out_kind,
                      inp["margin_lo"], inp["margin_hi"], hp, hc, d("lam"), d("beta_sky"), inp["orbit"], tdi, ws)
     torch.cuda.synchronize()
-    return hp.cpu().numpy(), hc.cpu().numpy(), ws.view(B, 6, N).cpu().numpy(), tdi.cpu().numpy()
+    return hp.cpu().numpy(), hc.cpu().numpy(), ws[:B * 6 * N].view(B, 6, N).cpu().numpy(), tdi.cpu().numpy()
 
 
 def _orc_chain(orc, inp, gen=20, out_kind=1, **kw):
