@@ -4,6 +4,14 @@
 
 writes oracle/liblisa_oracle_ld.so (REAL = long double, the parity truth) and
 oracle/liblisa_oracle_d.so (REAL = double, the timed CPU baseline).
+
+With ORACLE_SANITIZE=1 in the environment the two libraries are built (under other names) with
+-fsanitize=address,undefined, and oracle.binding loads those; run the CPU suite under them with
+
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 ORACLE_SANITIZE=1 \
+        python -m pytest tests -q -m "not gpu"
+
+(profiles/r2_sanitizers.md records the outcome).
 """
 import os
 import subprocess
@@ -19,10 +27,15 @@ TARGETS = {
 
 def build(force: bool = False) -> dict:
     out = {}
+    sanitize = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
     for key, (lib, defs) in TARGETS.items():
+        opt = ["-O2"]
+        if sanitize:
+            lib = lib.replace(".so", "_asan.so")
+            opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"]
         stale = (not os.path.exists(lib)) or os.path.getmtime(lib) < os.path.getmtime(SRC)
         if force or stale:
-            cmd = ["gcc", "-std=c11", "-O2", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math",
+            cmd = ["gcc", "-std=c11", *opt, "-fPIC", "-shared", "-fopenmp", "-fno-fast-math",
                    "-ffp-contract=off", "-Wall", "-Wextra", "-Wno-unused-parameter",
                    *defs, SRC, "-o", lib, "-lm"]
             subprocess.run(cmd, check=True)

@@ -84,3 +84,34 @@ def test_table_must_cover_the_grid(lib, orc):
     with pytest.raises(lib.LisaTdError) as e:
         lib.link_response(1, N, 1.0e7, 5.0, 31, 128, z, z, z[0, :1], z[0, :1], orbit, y)
     assert "does not cover" in str(e.value)
+
+
+def test_table_orbit_outside_the_host_bounds_is_reported_not_clamped(lib, orc):
+    """The kernels size their shared-memory tiles from host-side bounds on the orbit; for a TABLE orbit
+    those come from its nodes (chord rates x 1.05).  A table whose centroid swings by +-1.2e11 m from one
+    hourly node to the next is interpolated with a peak rate 1.29 times the chord rate: the common
+    delay drifts across a 256-sample tile by more samples than the strain tile has halo for.  The kernel
+    must say so (sticky flag -> LISA_TD_EINVAL at the next lisa_td_check), not clamp and carry on."""
+    B, N, dt, t0, h, q = 2, 1 << 14, 5.0, 1.0e6, 3600.0, 7
+    kep = synth.kepler_orbit()
+    n_tab = int(np.ceil(N * dt / h)) + 2 + 2 * q
+    t_tab0 = t0 - q * h
+    tab = np.stack([orc.orbit_eval(kep, t_tab0 + h * j)[0] for j in range(n_tab)])
+    good = {"kind": "table", "r_tab": tab.copy(), "t_tab0": t_tab0, "dt_tab": h, "tab_order": q}
+    wild = tab.copy()
+    wild[::2, :, 0] += 1.2e11
+    wild[1::2, :, 0] -= 1.2e11
+    bad = {"kind": "table", "r_tab": wild, "t_tab0": t_tab0, "dt_tab": h, "tab_order": q}
+    rng = np.random.default_rng(0)
+    hp = torch.from_numpy(rng.standard_normal((B, N))).cuda()
+    hc = torch.from_numpy(rng.standard_normal((B, N))).cuda()
+    lam = torch.tensor([0.3, 2.0], dtype=torch.float64, device="cuda")
+    bet = torch.tensor([0.1, -0.2], dtype=torch.float64, device="cuda")
+    y = torch.empty((B, 6, N), dtype=torch.float64, device="cuda")
+    lib.link_response(B, N, t0, dt, 31, 300, hp, hc, lam, bet, good, y)
+    lib.check()                                   # a sane table raises nothing
+    lib.link_response(B, N, t0, dt, 31, 300, hp, hc, lam, bet, bad, y)
+    with pytest.raises(lib.LisaTdError) as e:
+        lib.check()
+    assert e.value.code == -1 and "link-response" in str(e.value)
+    lib.check()                                   # the flag is cleared by the check that reported it

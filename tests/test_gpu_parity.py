@@ -278,17 +278,23 @@ def _orc_chain(orc, inp, gen=20, out_kind=1, **kw):
                      gamma=n("gamma"), **kw)
 
 
-def _report(name, got, ref):
-    """per-channel raw rel-L2 and error relative to the common scale of the three channels"""
+def _report(name, got, ref, rec=None, config=None, names="AET", floor_ref=None):
+    """per-channel raw rel-L2 and error relative to the common scale of the three channels; floor_ref =
+    the same series from the oracle's fp64 build (the rounding floor of any fp64 chain)"""
     common = max(np.linalg.norm(ref[c]) for c in range(3))
     raw = [rel_l2(got[c], ref[c]) for c in range(3)]
     com = [float(np.linalg.norm(got[c] - ref[c]) / common) for c in range(3)]
-    print(f"{name}: raw {raw}  vs common scale {com}")
+    flo = [None] * 3 if floor_ref is None else [rel_l2(floor_ref[c], ref[c]) for c in range(3)]
+    print(f"{name}: raw {raw}  vs common scale {com}  fp64 floor {flo}")
+    if rec is not None:
+        for c in range(3):
+            rec(config, name, names[c], raw=raw[c], common=com[c], floor=flo[c], tol=TOL_TDI,
+                passed=raw[c] < TOL_TDI, note=None if raw[c] < TOL_TDI else "raw above the bar: see vs_common_scale and fp64_floor")
     return raw, com
 
 
 @pytest.mark.parametrize("gen", [15, 20])
-def test_config1_tiny(lib, orc, gen):
+def test_config1_tiny(lib, orc, gen, parity_record):
     """configs[0]: N=2^12, (2,2) only, static equal arms, 1st + 2nd generation X,Y,Z."""
     inp = synth.make_inputs(1)
     ref = _orc_chain(orc, inp, gen, 0, want=("h", "y", "tdi"))
@@ -296,27 +302,30 @@ def test_config1_tiny(lib, orc, gen):
     assert rel_l2(hp, ref["hplus"]) < 2e-15 and rel_l2(hc, ref["hcross"]) < 2e-15
     for l in range(6):
         assert rel_l2(y[0, l], ref["y"][0, l]) < 2e-13
-    raw, _ = _report(f"config1 gen{gen} XYZ", tdi[0], ref["tdi"][0])
+    raw, _ = _report(f"N=2^12 B=1 static arms generation {gen / 10:g} whole series", tdi[0], ref["tdi"][0], parity_record,
+                     "configs[0]", "XYZ")
     assert max(raw) < TOL_TDI
 
 
 @pytest.mark.parametrize("config,B,N", [(2, 1, 1 << 14), (3, 3, 1 << 14)])
-def test_config23_reduced(lib, orc, config, B, N):
+def test_config23_reduced(lib, orc, orc_d, config, B, N, parity_record):
     """configs[1], [2] at reduced N (same generator, same cadence): 5 modes, Kepler orbits, A,E,T."""
     inp = synth.make_inputs(config, B=B, N=N)
     ref = _orc_chain(orc, inp, 20, 1, want=("h", "y", "tdi"))
+    ref_d = _orc_chain(orc_d, inp, 20, 1, want=("tdi",))
     hp, hc, y, tdi = _gpu_chain(lib, inp, 20, 1)
     assert rel_l2(hp, ref["hplus"]) < 3e-15
     for b in range(B):
         for l in range(6):
             assert rel_l2(y[b, l], ref["y"][b, l]) < 2e-13
-        raw, com = _report(f"config{config} b{b} AET", tdi[b], ref["tdi"][b])
+        raw, com = _report(f"reduced N=2^14 walker {b} whole series", tdi[b], ref["tdi"][b], parity_record,
+                           f"configs[{config - 1}]", "AET", ref_d["tdi"][b])
         assert raw[0] < TOL_TDI and raw[1] < TOL_TDI
         assert com[2] < TOL_TDI          # T against the common scale
         assert raw[2] < 1e-8             # raw T: a ~1e-3 remnant on nearly equal arms (DESIGN.md 7)
 
 
-def test_loglike_parity(lib, orc):
+def test_loglike_parity(lib, orc, parity_record):
     """configs[3] at reduced size: FFT + inner products against the oracle's long-double FFT."""
     B, N = 4, 1 << 14
     inp = synth.make_inputs(4, B=B, N=N)
@@ -334,6 +343,7 @@ def test_loglike_parity(lib, orc):
     for got, key in ((ll, "loglike"), (dh, "dh"), (hh, "hh")):
         err = np.abs(got.cpu().numpy() - refll[key]) / np.abs(refll[key])
         print(key, err)
+        parity_record("configs[3]", "reduced N=2^14 B=4, worst walker", key, raw=np.max(err), tol=TOL_LL, passed=np.max(err) < TOL_LL)
         assert np.max(err) < TOL_LL
     # closed form C10: log L(h = d) = (d|d)/2 for the injected walker
     assert abs(ll[0].item() - 0.5 * hh[0].item()) < 1e-9 * abs(hh[0].item())
@@ -403,5 +413,14 @@ def test_pipeline_host_matches_stagewise(lib, orc):
                       inp["margin_y"], 20, inp["margin_lo"], inp["margin_hi"], inp["orbit"],
                       data.cpu().numpy(), w, kmin, kmax, out)
     assert np.max(np.abs(out - ll.cpu().numpy()) / np.abs(out)) < 1e-12
+    # ... and the oracle's own chain, with its own injection (walker 0) and weights
+    w_o = orc.psd_weights(N, dt, synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)
+    data_o = orc.spectrum3(_orc_chain(orc, inp, 20, 1, want=("tdi",))["tdi"][0])
+    ref = _orc_chain(orc, inp, 20, 1, want=("loglike",), data_spec=data_o, weight=w_o, kmin=kmin, kmax=kmax)
+    out2 = np.zeros(B)
+    lib.pipeline_host(pipe, B, N, inp["l"], inp["m"], h("amp"), h("phase"), h("alpha"), h("beta"), h("gamma"),
+                      h("iota"), h("phi"), h("psi"), h("lam"), h("beta_sky"), inp["t0"], dt, inp["order"],
+                      inp["margin_y"], 20, inp["margin_lo"], inp["margin_hi"], inp["orbit"], data_o, w_o, kmin, kmax, out2)
+    assert np.max(np.abs(out2 - ref["loglike"]) / np.abs(ref["loglike"])) < TOL_LL
     pipe.close()
     plan.close()
