@@ -47,8 +47,13 @@ K2_GEOM = 150
 K2_OPS = K2_SWEEP + K2_GEOM            # 1725 ops = 3450 flop per walker-sample
 K2_BYTES = 16 + 48                     # h+,hx in, six links out
 # dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch at this workload
-# (ncu --set full capture summarised in profiles/r1_s3_k2_k3.md: 1.074 GB read + 3.188 GB written)
-K2_TRAFFIC_BYTES = 4.262e9
+# (ncu --set full capture summarised in profiles/r2_s1.md: 1.07 GB read + 3.17 GB written)
+K2_TRAFFIC_BYTES = 4.24e9
+# K3 (TDI-2, A,E,T): 12 (channel, series) pairs x 44 merged-stencil taps = 528 MACs per walker-sample
+# (the 8x8x4 tiles of the banded product issue 624); 48 B of links in, 24 B out
+K3_OPS = 528
+K3_BYTES = 48 + 24
+K1_OPS_EXECUTED = 334                  # fp64 instructions per sample of the five-mode kernel (ncu)
 
 
 def parse():
@@ -403,6 +408,36 @@ def run_ours(args):
                    "s2_hbm_gbs": 64.0 * B * N / (o1_ms2 * 1e-3) / 1e9, "s3_hbm_gbs": 72.0 * B * N / (o1_ms3 * 1e-3) / 1e9,
                    "hbm_bytes_per_walker_sample": {"s2": 64, "s3": 72},
                    "cite": "PAPER.md:209 (linear interpolation); SURVEY 8(d)"}
+    # ---- the fused response+TDI kernel north_star sketches, bounded by measurement:
+    # a block that keeps the six links of a time tile in shared memory must compute them on the tile PLUS the
+    # reach of the merged TDI stencils (51 samples at order 31, generation 2).  At the largest tile whose links
+    # fit in shared memory for 8 walkers (256 outputs -> 307 link samples) its link-response phase is the
+    # committed K2 on 307/256 as many samples; its TDI phase is the same banded DMMA product as k3_tdi_mma.
+    Nf = ((N * 307 + 255) // 256 + 1) // 2 * 2
+    hp_f = torch.zeros((B, Nf), dtype=f64, device=device)
+    hc_f = torch.zeros((B, Nf), dtype=f64, device=device)
+    hp_f[:, :N] = hp
+    hc_f[:, :N] = hc
+    y_f = torch.empty((B, 6, Nf), dtype=f64, device=device)
+
+    def fused_k2_phase():
+        lib.link_response(B, Nf, t0, dt, ORDER, inp["margin_y"], hp_f, hc_f, g("lam"), g("beta_sky"), inp["orbit"], y_f)
+    for _ in range(3):
+        fused_k2_phase()
+    fb = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    fb[0].record()
+    for _ in range(5):
+        fused_k2_phase()
+    fb[1].record()
+    torch.cuda.synchronize()
+    ms_k2_fused = fb[0].elapsed_time(fb[1]) / 5
+    del hp_f, hc_f, y_f
+    fused_info = {"ms_k2_on_tile_plus_stencil_reach": ms_k2_fused, "ms_k2": stage_ms["S2_link_response"],
+                  "ms_k3": stage_ms["S3_tdi2"], "ms_unfused_k2_plus_k3": stage_ms["S2_link_response"] + stage_ms["S3_tdi2"],
+                  "ms_fused_lower_bound": ms_k2_fused + stage_ms["S3_tdi2"],
+                  "reading": "lower bound of a fused kernel with 256-output tiles = K2 on 307/256 of the samples + the same DMMA "
+                             "product; the HBM round trip it would save (6.4 GB) is hidden under fp64 work in the unfused path",
+                  "cite": "north_star 'fused TDI2 delay-and-sum kept in shared memory'; DESIGN.md section 9"}
     s2(); s3()
     torch.cuda.synchronize()
     fisher_info = {"D": D, "walkers": D + 1, "ms_per_matrix": fe[0].elapsed_time(fe[1]) / 5,
@@ -428,6 +463,26 @@ def run_ours(args):
         "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback",
         "hbm_frac": K2_BYTES * ws / (k2_ms * 1e-3) / 1e9 / hbm_peak,
     }
+
+    k3_ms = stage_ms["S3_tdi2"]
+    roofline["other_kernels"] = {
+        "k3_tdi (anchor tables + mma + fix-up)": {
+            "bound": "alu (fp64 tensor path, same units)", "ms_per_launch": k3_ms, "ops_per_walker_sample": K3_OPS,
+            "achieved": 2 * K3_OPS * ws / (k3_ms * 1e-3) / 1e12, "frac": 2 * K3_OPS * ws / (k3_ms * 1e-3) / 1e12 / dfma_peak_tflops,
+            "hbm_achieved_gbs": K3_BYTES * ws / (k3_ms * 1e-3) / 1e9},
+        "k1_modes_to_pol": {
+            "bound": "alu and hbm, about equally", "ms_per_launch": stage_ms["S1_modes_to_pol"],
+            "executed_ops_per_sample": K1_OPS_EXECUTED,
+            "frac_alu_executed": 2 * K1_OPS_EXECUTED * ws / (stage_ms["S1_modes_to_pol"] * 1e-3) / 1e12 / dfma_peak_tflops,
+            "hbm_achieved_gbs": 120.0 * ws / (stage_ms["S1_modes_to_pol"] * 1e-3) / 1e9,
+            "hbm_frac": 120.0 * ws / (stage_ms["S1_modes_to_pol"] * 1e-3) / 1e9 / hbm_peak},
+        "whole_step": {
+            "credited_ops_per_walker_sample": K1_OPS_EXECUTED + K2_OPS + K3_OPS,
+            "frac_of_fp64_peak": 2 * (K1_OPS_EXECUTED + K2_OPS + K3_OPS) * ws / (ms_per_step * 1e-3) / 1e12 / dfma_peak_tflops},
+    }
+    # the 0.76 of K2 credits 1725 ops, 98 % of what the kernel executes; the count SURVEY 8(d) priced
+    # (576 stencil FMAs + 100 geometry, without the nine walker-dependent coefficient sets) gives:
+    roofline["frac_survey_priced_ops"] = 2 * (576 + 100) * ws / (k2_ms * 1e-3) / 1e12 / dfma_peak_tflops
 
     # ---- end to end through the host API (pinned host buffers, copies inside the timed region)
     e2e = None
@@ -493,12 +548,13 @@ def run_ours(args):
                    "l2": "inputs (6.8 GB per step) and every intermediate exceed the 126 MB L2",
                    "parallelism": f"walker-split x{world}, no collective"},
         "samples_per_s": value * N, "stage_ms": stage_ms, "roofline": roofline, "cpu_baseline": cpu_baseline,
-        "e2e": e2e, "gpu_launches": 5 * args.steps, "launches_per_step": {
-            "k1_modes_to_pol_std5_tma": 1, "k2_link_response": 1, "k3_tdi_mma": 1, "k5_inner_partial": 1,
-            "k5_inner_final": 1, "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
+        "e2e": e2e, "gpu_launches": 7 * args.steps, "launches_per_step": {
+            "k1_modes_to_pol_std5_tma": 1, "k2_link_response": 1, "k3_anchor_tables": 1, "k3_tdi_mma": 1,
+            "k3_tdi_fixup": 1, "k5_inner_partial": 1, "k5_inner_final": 1,
+            "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops, "fp64_pipes": pipes,
         "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info,
-                 "order1": order1_info},
+                 "order1": order1_info, "fused_bound": fused_info},
     }
     print(json.dumps(line))
     plan.close()

@@ -623,17 +623,25 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
       double* xsc = xs + (size_t)buf * (3 * K3_TS * K3_XS);
       // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
       const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
-      double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
+      // four independent accumulator chains per warp (two walker groups x even / odd k-steps): with
+      // three warps per scheduler that is twelve DMMAs in flight against the latency of one
+      double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0, e00 = 0.0, e01 = 0.0, e10 = 0.0, e11 = 0.0;
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const double* y0 = yb + ser[q] * TW;
         const double* y1 = y0 + 8 * 6 * TW;
 #pragma unroll
         for (int ks = 0; ks < KSTEPS; ++ks) {
-          dmma884(d00, d01, A[q][ks], y0[4 * ks]);
-          dmma884(d10, d11, A[q][ks], y1[4 * ks]);
+          if ((ks & 1) == 0) {
+            dmma884(d00, d01, A[q][ks], y0[4 * ks]);
+            dmma884(d10, d11, A[q][ks], y1[4 * ks]);
+          } else {
+            dmma884(e00, e01, A[q][ks], y0[4 * ks]);
+            dmma884(e10, e11, A[q][ks], y1[4 * ks]);
+          }
         }
       }
+      d00 += e00; d01 += e01; d10 += e10; d11 += e11;
       {
         double* xr = xsc + (size_t)(ch * K3_TS + rb * 8 + r) * K3_XS + 2 * kk;
         xr[0] = d00; xr[1] = d01; xr[8] = d10; xr[9] = d11;
