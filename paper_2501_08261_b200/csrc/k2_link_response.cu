@@ -60,16 +60,21 @@ __device__ __forceinline__ void read_pair2(const double2* __restrict__ xe, const
   const double Ka = ceil(Dc[0] + Dla), Kb = ceil(Dc[1] + Dlb);
   const double epsa = (Ka - Dc[0]) - Dla, epsb = (Kb - Dc[1]) - Dlb;
   // the halo (sized from host-side bounds on the orbit) must keep every window inside the tile;
-  // if it does not, say so (the clamp is for memory safety only: the value is then wrong)
-  int ea = ea0 - (int)Ka, eb = ea0 + 1 - (int)Kb;
-  if (ea < elo || ea > ehi || eb < elo || eb > ehi + 1) {
+  // if it does not, say so (the clamp is for memory safety only: the value is then wrong).
+  // One unsigned compare per read on the hot path: ea in [elo, ehi].
+  int ea = ea0 - (int)Ka;
+  if ((unsigned)(ea - elo) > (unsigned)(ehi - elo)) {
     raise_error(p.err, DEVERR_K2_WINDOW);
     ea = max(elo, min(ea, ehi));
-    eb = max(elo, min(eb, ehi));
   }
   if (Ka == Kb) {
     lagrange_dot2h_x2<HT>(epsa, epsb, p.half, p.ls, xe, xo, ea, vp, vc);
-  } else {
+  } else {  // cold path: the two samples of the pair have different integer delays
+    int eb = ea0 + 1 - (int)Kb;
+    if (eb < elo || eb > ehi + 1) {
+      raise_error(p.err, DEVERR_K2_WINDOW);
+      eb = max(elo, min(eb, ehi));
+    }
     lagrange_dot2h_split(epsa, p.half, p.ls, xe, xo, ea, vp[0], vc[0]);
     lagrange_dot2h_split(epsb, p.half, p.ls, xe, xo, eb, vp[1], vc[1]);
   }

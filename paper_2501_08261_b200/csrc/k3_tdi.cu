@@ -244,15 +244,17 @@ __global__ void __launch_bounds__(256) k3_tdi_generic(const K3Params p) {
 }
 
 // Fix-up pass behind the merged-stencil kernel: recomputes, sample by sample, the tiles of `tile`
-// samples that k3_anchor_tables listed (list[0] = count, list[1..] = tile indices).  Work item =
-// (listed tile, group of 8 walkers), thread = (sample, walker); blocks without an item leave at once.
+// samples (an anchor group, a divisor of 256) that k3_anchor_tables listed (list[0] = count,
+// list[1..] = group indices).  Work item = (listed group, 256 / tile walkers), thread = (sample,
+// walker); blocks without an item leave at once.
 template <int HT>
 __global__ void __launch_bounds__(256) k3_tdi_fixup(const K3Params p, const int* __restrict__ list, const int tile) {
-  const int groups = (p.B + 7) / 8;
+  const int wpi = 256 / tile;  // walkers per item
+  const int groups = (p.B + wpi - 1) / wpi;
   const int items = list[0] * groups;
   for (int item = blockIdx.x; item < items; item += gridDim.x) {
     const long long n = (long long)list[1 + item / groups] * tile + (threadIdx.x % tile);
-    const int b = (item % groups) * 8 + threadIdx.x / tile;
+    const int b = (item % groups) * wpi + threadIdx.x / tile;
     if (n < p.N && b < p.B) k3_generic_sample<HT>(p, n, b);
   }
 }
@@ -271,11 +273,11 @@ __global__ void __launch_bounds__(256) k3_tdi_fixup(const K3Params p, const int*
 // each.  Walkers stream through shared memory in chunks of 16, one 2-D tensor-map TMA copy per
 // chunk (double buffered, mbarrier completion); X,Y,Z of a chunk meet in shared memory for A,E,T.
 //
-// Merged stencils from three anchors.  Within a tile no integer delay changes (checked), so every
-// tap of the merged stencil is a smooth function of the sample: it is evaluated EXACTLY at the
-// anchor samples 0, 16, 32 of the tile (3 x 48 coefficient sweeps instead of 32 x 48) and every
-// row gets the quadratic through the anchors (truncation |f'''| 16^3 0.064 < 1e-16 of a tap for
-// |dD/dn| < 1e-6).  Tiles where an integer delay does change (one in ~1e4), where
+// Merged stencils from three anchors.  Within a group of four tiles (128 samples) no integer delay
+// changes (checked), so every tap of the merged stencil is a smooth function of the sample: it is
+// evaluated EXACTLY at the anchor samples 0, 64, 128 of the group (3 x 48 coefficient sweeps
+// instead of 128 x 48) and every row gets the quadratic through the anchors (truncation
+// |f'''| 64^3 0.064 ~ 5e-15 of a tap on a heliocentric orbit).  Tiles where an integer delay does change (one in ~1e4), where
 // the delay is not smooth enough, or that straddle a node of a tabulated orbit are flagged and
 // listed, and recomputed sample by sample by a fix-up pass (k3_tdi_fixup).
 //
@@ -293,12 +295,14 @@ constexpr int K3_THREADS = K3_TS * K3_PAIRS;  // 384: warp = (channel, row block
 // parabola through samples 0, 16, 32: ~10x the rounding noise of a delay of ~12 samples formed from
 // six square roots (4e-15 rms), far below anything that matters for a tap (|dc/deps| ~ 3)
 constexpr double K3_SMOOTH_TOL = 1e-13;
-constexpr int K3_TAB_TILES = 2;               // tiles per block of k3_anchor_tables
+constexpr int K3_TAB_TILES = 2;               // anchor groups per block of k3_anchor_tables
 constexpr int K3_TAB_THREADS = 96;
 constexpr int K3_RB = K3_TS / 8;              // 8-row blocks per tile
 constexpr int K3_WC = 16;                     // walkers per shared-memory chunk (two MMA N-blocks)
 constexpr int K3_XS = K3_WC + 1;              // row stride of the X,Y,Z exchange buffer
-constexpr int K3_AH = K3_TS / 2;              // anchor spacing: anchors at tile samples 0, 16, 32
+constexpr int K3_GT = 4;                      // tiles per anchor group: one table serves 128 samples
+constexpr int K3_GS = K3_GT * K3_TS;          // samples per anchor group
+constexpr int K3_AH = K3_GS / 2;              // anchor spacing: anchors at group samples 0, 64, 128
 
 __device__ __forceinline__ void cp_async8_zfill(void* smem, const void* gmem, bool valid) {
   unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -397,13 +401,14 @@ struct K3Geom {
 
 __device__ __forceinline__ int k3_anchor_sample(int a) { return a == 3 ? K3_AH / 2 : a * K3_AH; }
 
-// Anchor tables.  Block = K3_TAB_TILES tiles.  Phase A: the delays of every tile at its anchor
-// samples n0, n0 + 16, n0 + 32 and at the check sample n0 + 8.  Phase B: thread = (tile, pair,
+// Anchor tables.  Block = K3_TAB_TILES anchor groups (called "tiles" below; a group is K3_GS = 128
+// samples = four MMA tiles).  Phase A: the delays of every group at its anchor samples n0,
+// n0 + 64, n0 + 128 and at the check sample n0 + 32.  Phase B: thread = (tile, pair,
 // anchor) sweeps the terms of its pair into one row of WIN taps.  A tile is flagged `split` (the MMA
 // kernel then takes the exact per-row path) if an integer delay differs between its anchors, if
-// the delay is not a parabola in the sample to 1e-13 samples (checked at sample 8, where the cubic
+// the delay is not a parabola in the sample to 1e-13 samples (checked at sample 32, where the cubic
 // term equals the largest interpolation error over the tile), or if it straddles a node of a
-// tabulated orbit.  tab: [n_tiles][12][3][QS], flag in slot QFLAG of row 0; flagged tiles are also
+// tabulated orbit.  tab: [n_groups][12][3][QS], flag in slot QFLAG of row 0; flagged groups are also
 // appended to `list` (count, then tile indices) for the fix-up pass.
 template <int H, int WIN>
 __global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_constant__ K3Params p, double* __restrict__ tab,
@@ -421,10 +426,10 @@ __global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_
   if (tid < T) {
     int sp = 0;
     if (p.orb.kind == 2) {  // a tabulated orbit is a different polynomial on either side of a table node
-      const long long n0 = (long long)(tile0 + tid) * K3_TS;
+      const long long n0 = (long long)(tile0 + tid) * K3_GS;
       const double reach = p.orb.nested ? 8.0 * p.orb.max_L : 0.0;
       const double ua = (fma((double)n0, p.dt, p.t0) - reach - p.orb.t_tab0) * p.orb.inv_dt_tab;
-      const double ub = (fma((double)(n0 + K3_TS), p.dt, p.t0) - p.orb.t_tab0) * p.orb.inv_dt_tab;
+      const double ub = (fma((double)(n0 + K3_GS), p.dt, p.t0) - p.orb.t_tab0) * p.orb.inv_dt_tab;
       sp = floor(ua) != floor(ub);
     }
     split[tid] = sp;
@@ -435,7 +440,7 @@ __global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_
     if (p.orb.kind == 1) {
       if (tid < T * NA * 3) {
         const int tl = tid / (NA * 3), a = (tid / 3) % NA, k = tid % 3;
-        const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+        const long long n = (long long)(tile0 + tl) * K3_GS + k3_anchor_sample(a);
         double L[6];
         orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0) - (double)k * hq, L);
 #pragma unroll
@@ -445,7 +450,7 @@ __global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_
     }
     if (tid < T * NA * 6) {
       const int tl = tid / (NA * 6), a = (tid / 6) % NA, cp = tid % 6;  // cp = channel * 2 + path
-      const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+      const long long n = (long long)(tile0 + tl) * K3_GS + k3_anchor_sample(a);
       double tau[8];
       if (p.orb.kind == 1) chain_delays_quad(Lq + (tl * NA + a) * 18, 1.0 / hq, p.path[cp >> 1][cp & 1], tau);
       else chain_delays(p.orb, fma((double)n, p.dt, p.t0), p.path[cp >> 1][cp & 1], tau);
@@ -454,7 +459,7 @@ __global__ void __launch_bounds__(K3_TAB_THREADS) k3_anchor_tables(const __grid_
     }
   } else if (tid < T * NA) {
     const int tl = tid / NA, a = tid % NA;
-    const long long n = (long long)(tile0 + tl) * K3_TS + k3_anchor_sample(a);
+    const long long n = (long long)(tile0 + tl) * K3_GS + k3_anchor_sample(a);
     double L[6];
     orbit_arm_times(p.orb, fma((double)n, p.dt, p.t0), L);
 #pragma unroll
@@ -533,7 +538,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
   auto tile_n0 = [&](int it) { return tile_id(it) * K3_TS; };
   auto fetch_table = [&](int it) {  // thread 0: anchor table of this block's tile `it` into buffer it & 1
     mbar_arrive_expect_tx(&tbar[it & 1], (unsigned)(G::QBUF * sizeof(double)));
-    tma_load_1d(qtab + (it & 1) * G::QBUF, tab + (size_t)tile_id(it) * G::QBUF, (unsigned)(G::QBUF * sizeof(double)), &tbar[it & 1]);
+    tma_load_1d(qtab + (it & 1) * G::QBUF, tab + (size_t)(tile_id(it) / K3_GT) * G::QBUF, (unsigned)(G::QBUF * sizeof(double)), &tbar[it & 1]);
   };
   if (threadIdx.x == 0 && my_tiles > 0) fetch_table(0);
 
@@ -588,8 +593,8 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
     // behind this kernel overwrites its outputs)
     double A[4][KSTEPS];
     {
-      // weights of the three anchors at this lane's row (quadratic through samples 0, 16, 32)
-      const double u = (double)(rb * 8 + r) * (1.0 / K3_AH);
+      // weights of the three anchors at this lane's row (quadratic through samples 0, 64, 128 of the group)
+      const double u = (double)((int)(tile_id(it) % K3_GT) * K3_TS + rb * 8 + r) * (1.0 / K3_AH);
       const double w0 = 0.5 * (u - 1.0) * (u - 2.0), w1 = u * (2.0 - u), w2 = 0.5 * u * (u - 1.0);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
@@ -699,12 +704,12 @@ static EncodeTiledFn encode_tiled_fn() {
 
 // bytes of workspace run_tdi needs for N samples: the anchor tables (sized for the widest window),
 // then the list of flagged tiles
-static long long tdi_table_bytes(long long n_tiles) {
-  return ((n_tiles * (long long)K3Geom<16, 48>::QBUF * (long long)sizeof(double)) + 255) / 256 * 256;
+static long long tdi_table_bytes(long long n_groups) {
+  return ((n_groups * (long long)K3Geom<16, 48>::QBUF * (long long)sizeof(double)) + 255) / 256 * 256;
 }
 long long tdi_workspace_bytes(long long N) {
-  const long long n_tiles = (N + K3_TS - 1) / K3_TS;
-  return tdi_table_bytes(n_tiles) + ((n_tiles + 1) * (long long)sizeof(int) + 255) / 256 * 256;
+  const long long n_groups = (N + K3_GS - 1) / K3_GS;
+  return tdi_table_bytes(n_groups) + ((n_groups + 1) * (long long)sizeof(int) + 255) / 256 * 256;
 }
 
 template <int H, int WIN>
@@ -729,9 +734,10 @@ static int launch_mma(const K3Params& p, double* tab, cudaStream_t st) {
   }
   const long long n_tiles = (p.N + K3_TS - 1) / K3_TS;
   // 1. anchor stencils of every tile (walker-independent)
-  int* list = reinterpret_cast<int*>(reinterpret_cast<char*>(tab) + tdi_table_bytes(n_tiles));
+  const long long n_groups = (p.N + K3_GS - 1) / K3_GS;
+  int* list = reinterpret_cast<int*>(reinterpret_cast<char*>(tab) + tdi_table_bytes(n_groups));
   LISA_CUDA(cudaMemsetAsync(list, 0, sizeof(int), st));
-  k3_anchor_tables<H, WIN><<<(unsigned)((n_tiles + K3_TAB_TILES - 1) / K3_TAB_TILES), K3_TAB_THREADS, 0, st>>>(p, tab, list, (int)n_tiles);
+  k3_anchor_tables<H, WIN><<<(unsigned)((n_groups + K3_TAB_TILES - 1) / K3_TAB_TILES), K3_TAB_THREADS, 0, st>>>(p, tab, list, (int)n_groups);
   LISA_LAUNCH_CHECK("k3_anchor_tables");
   // 2. persistent MMA blocks: one (two at order 1) per SM, each walking over tiles blockIdx.x + i gridDim.x
   LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
@@ -740,7 +746,7 @@ static int launch_mma(const K3Params& p, double* tab, cudaStream_t st) {
   k3_tdi_mma<H, WIN><<<grid, K3_THREADS, G::SMEM, st>>>(p, tmap, use_tma, tab, (int)n_tiles);
   LISA_LAUNCH_CHECK("k3_tdi_mma");
   // 3. fix-up: the flagged tiles, sample by sample (threads of other tiles leave at once)
-  k3_tdi_fixup<H><<<2 * sm_count(), 256, 0, st>>>(p, list, K3_TS);
+  k3_tdi_fixup<H><<<2 * sm_count(), 256, 0, st>>>(p, list, K3_GS);
   LISA_LAUNCH_CHECK("k3_tdi_fixup");
   return LISA_TD_OK;
 }

@@ -72,7 +72,7 @@ def test_argument_validation_happens_before_any_launch(lib):
     # loglike: band outside the spectrum, NULL plan
     assert L.lisa_td_loglike(None, 1, 16, fake, fake, fake, 0, 4, fake, None, None, None) == -1
     # workspace size helper
-    assert L.lisa_td_response_tdi_workspace_bytes(2, 1024) >= 2 * 6 * 1024 * 8 + 32 * 12 * 3 * 44 * 8  # links + anchor tables
+    assert L.lisa_td_response_tdi_workspace_bytes(2, 1024) >= 2 * 6 * 1024 * 8 + 8 * 12 * 3 * 44 * 8  # links + anchor tables (one per 128 samples)
 
 
 def test_combined_calls_add_the_link_margin_to_the_tdi_margins(lib):
