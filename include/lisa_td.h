@@ -163,16 +163,21 @@ LISA_TD_API int lisa_td_laser_links(long long N, double t0, double dt, int order
  * (p+1)/2 (3 Lmax for generation 15) and margin_hi >= (p+1)/2.  If y came from
  * lisa_td_link_response with margin_y, the caller must ADD margin_y to both (reading A7: TDI must
  * not interpolate across the zeroed edge of y); this call cannot know margin_y and does not check
- * that, lisa_td_response_tdi and lisa_td_pipeline_host do. */
+ * that, lisa_td_response_tdi and lisa_td_pipeline_host do.
+ * Temporary memory: at orders 1 and 31 the walker-independent merged stencils of the call (13 KB
+ * per 128 samples, plus a list of sample groups to recompute one by one) are drawn from the device's
+ * stream-ordered memory pool (cudaMallocAsync / cudaFreeAsync on `stream`): no synchronisation, the
+ * memory is released in stream order and the pool keeps the pages for the next call.  The call stays
+ * capturable into a CUDA graph.  lisa_td_response_tdi keeps them in the caller's workspace instead. */
 LISA_TD_API int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
                  long long margin_lo, long long margin_hi, const double* y,
                  const lisa_td_orbit* orbit_host, double* tdi, void* stream);
 
 /* S2+S3 in one call: h+,hx -> tdi.  This is lisa_td_link_response into `workspace` followed by
  * lisa_td_tdi2 from it: all six links of all B walkers make one round trip through HBM ([B][6][N]
- * doubles = 48 B N bytes, the size lisa_td_response_tdi_workspace_bytes returns), they just never
- * appear in a caller array.  An on-chip fusion was prototyped and measured slower (DESIGN.md
- * section 9, profiles/r2_fused_prototype.md): both kernels are bound by fp64 arithmetic, not by the
+ * doubles = 48 B N bytes; lisa_td_response_tdi_workspace_bytes returns that plus the anchor
+ * tables of S3, ~100 B per sample), they just never appear in a caller array.  An on-chip fusion was prototyped and measured slower (DESIGN.md
+ * section 9, profiles/r2_s1.md): both kernels are bound by fp64 arithmetic, not by the
  * round trip.  Requires margin_lo >= margin_y + reach and margin_hi >= margin_y + (p+1)/2. */
 LISA_TD_API long long lisa_td_response_tdi_workspace_bytes(int B, long long N);
 LISA_TD_API int lisa_td_response_tdi(int B, long long N, double t0, double dt, int order, long long margin_y,

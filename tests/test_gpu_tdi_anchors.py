@@ -103,3 +103,18 @@ def test_anchored_rows_match_the_generic_kernel(lib):
     finally:
         lib.debug_force_generic(0)
     assert np.max(np.abs(a - b)) < 2e-14 * np.sqrt(np.mean(b ** 2)) * 10
+
+
+@pytest.mark.parametrize("N,B", [(70, 1), (130, 2), (257, 17), (1000, 16), (1153, 40)])
+def test_short_and_ragged_grids(lib, orc, N, B):
+    """fewer samples than one anchor group (128) or one MMA tile (32), odd N (cp.async path), grids that
+    end inside a group, walker counts around the chunk size of 16"""
+    rng = np.random.default_rng(N + B)
+    dt, order, t0 = 5.0, 31, 5.0e6
+    orbit = synth.kepler_orbit()
+    mlo, mhi = 28, 16
+    y = rng.standard_normal((B, 6, N))
+    for gen in (15, 20):
+        ref = orc.tdi(y, orbit, t0, dt, order, gen, 1, mlo, mhi)
+        got = _gpu_tdi(lib, y, orbit, t0, dt, order, gen, 1, mlo, mhi)
+        _assert_close(got, ref, mlo, mhi)
