@@ -304,6 +304,27 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    # ---- the same step through the one-call API (lisa_td_loglike_from_modes: S1..S5 from device inputs)
+    ws_fm = torch.empty(lib.loglike_from_modes_workspace_bytes(B, N) // 8, dtype=f64, device=device)
+    ll_fm = torch.empty(B, dtype=f64, device=device)
+
+    def one_call():
+        lib.loglike_from_modes(plan, B, N, inp["l"], inp["m"], g("amp"), g("phase"), g("alpha"), g("beta"), g("gamma"),
+                               g("iota"), g("phi"), g("psi"), g("lam"), g("beta_sky"), t0, dt, ORDER, inp["margin_y"], 20,
+                               inp["margin_lo"], inp["margin_hi"], inp["orbit"], data, weight, kmin, kmax, ll_fm, None, None,
+                               ws_fm)
+    for _ in range(3):
+        one_call()
+    oc = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    oc[0].record()
+    for _ in range(5):
+        one_call()
+    oc[1].record()
+    torch.cuda.synchronize()
+    one_call_info = {"ms_per_step": oc[0].elapsed_time(oc[1]) / 5, "api": "lisa_td_loglike_from_modes",
+                     "bit_identical_to_stagewise": bool(torch.equal(ll_fm, ll))}
+    del ws_fm
+
     # ---- batched finite-difference Fisher matrix, D = 15
     # parameters = 16 walkers (centre + 15 perturbed; the first 16 walkers of the batch, which
     # are 1e-3 perturbations of walker 0, stand in for them) through S1..S3 + lisa_td_fisher
@@ -557,7 +578,7 @@ def run_ours(args):
             "cufft (library)": "Z2Z length N/2, batch 192 (packed real input)"},
         "clocks": clocks, "loglike_walker0": loglike0, "dfma_peak_tflops_measured": dfma_peak_tflops, "fp64_pipes": pipes,
         "next": {"fisher": fisher_info, "up2": up2_info, "nested": nested_info, "channels": ch_info,
-                 "order1": order1_info, "fused_bound": fused_info},
+                 "order1": order1_info, "fused_bound": fused_info, "one_call": one_call_info},
     }
     print(json.dumps(line))
     plan.close()

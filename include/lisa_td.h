@@ -210,6 +210,24 @@ LISA_TD_API int lisa_td_loglike_channels(lisa_td_plan* plan, int B, long long N,
                              const double* data_spec, const double* weight, long long kmin, long long kmax,
                              double* loglike, double* dh, double* hh, void* stream);
 
+/* S1..S5 in one call from DEVICE inputs (the call a sampler makes per batch of walkers): modes ->
+ * h+,hx -> six links -> TDI A,E,T of the given generation -> FFT -> log L, enqueued on `stream`
+ * without synchronising.  Arguments as in lisa_td_modes_to_pol (no euler0), lisa_td_link_response,
+ * lisa_td_tdi2 and lisa_td_loglike; margins as in lisa_td_response_tdi.  Every intermediate lives in
+ * `workspace` (device, >= lisa_td_loglike_from_modes_workspace_bytes(B, N) bytes = 88 B N plus the
+ * anchor tables of S3; 5.9 GB at B = 64, N = 2^20).  The stages run one after the other on the one
+ * stream: every compute kernel of the path fills the register file of every SM, so chunking the
+ * batch over a second stream to hide the FFT was measured and does not pay. */
+LISA_TD_API long long lisa_td_loglike_from_modes_workspace_bytes(int B, long long N);
+LISA_TD_API int lisa_td_loglike_from_modes(lisa_td_plan* plan, int B, long long N, int n_modes, const int* l_host,
+                               const int* m_host, const double* amp, const double* phase, const double* alpha,
+                               const double* beta, const double* gamma, const double* iota, const double* phi,
+                               const double* psi, const double* lambda, const double* beta_sky, double t0,
+                               double dt, int order, long long margin_y, int generation, long long margin_lo,
+                               long long margin_hi, const lisa_td_orbit* orbit_host, const double* data_spec,
+                               const double* weight, long long kmin, long long kmax, double* loglike, double* dh,
+                               double* hh, void* workspace, long long workspace_bytes, void* stream);
+
 /* Fisher matrix by first-order finite differences ("The Fisher matrix is computed
  * from the derivatives of the likelihood function, using first-order finite differences";
  * reading A19 of DESIGN.md).  tdi: [D+1][3][N] (A,E,T): walker 0 is the centre theta, walker

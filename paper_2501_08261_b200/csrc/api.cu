@@ -575,6 +575,63 @@ int lisa_td_loglike(lisa_td_plan* plan, int B, long long N, const double* tdi,
   return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, (cudaStream_t)stream, 3);
 }
 
+// ---- S1..S5 from DEVICE inputs in one call
+static long long al256(long long v) { return (v + 255) / 256 * 256; }
+long long lisa_td_loglike_from_modes_workspace_bytes(int B, long long N) {
+  if (B <= 0 || N <= 0) return 0;
+  const long long d = (long long)sizeof(double);
+  // h+, hx [B][N] | y [B][6][N] | tdi [B][3][N] | anchor tables of S3
+  return 2 * al256(d * B * N) + al256(d * 6 * B * N) + al256(d * 3 * B * N) + tdi_workspace_bytes(N);
+}
+
+int lisa_td_loglike_from_modes(lisa_td_plan* plan, int B, long long N, int n_modes, const int* l_host, const int* m_host,
+                               const double* amp, const double* phase, const double* alpha, const double* beta,
+                               const double* gamma, const double* iota, const double* phi, const double* psi,
+                               const double* lambda, const double* beta_sky, double t0, double dt, int order,
+                               long long margin_y, int generation, long long margin_lo, long long margin_hi,
+                               const lisa_td_orbit* orbit_host, const double* data_spec, const double* weight,
+                               long long kmin, long long kmax, double* loglike, double* dh, double* hh, void* workspace,
+                               long long workspace_bytes, void* stream) {
+  const char* fn = "lisa_td_loglike_from_modes";
+  if (!plan) return set_error(LISA_TD_EINVAL, "%s: plan is NULL", fn);
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (n_modes <= 0 || n_modes > 16) return set_error(LISA_TD_EINVAL, "%s: n_modes must be in [1,16]", fn);
+  if (!l_host || !m_host) return set_error(LISA_TD_EINVAL, "%s: l_host / m_host is NULL", fn);
+  for (int k = 0; k < n_modes; ++k)
+    if (l_host[k] < 2 || l_host[k] > 8 || m_host[k] < -l_host[k] || m_host[k] > l_host[k])
+      return set_error(LISA_TD_EINVAL, "%s: mode %d = (%d,%d) outside 2<=l<=8, |m|<=l", fn, k, l_host[k], m_host[k]);
+  REQUIRE_PTR(fn, amp); REQUIRE_PTR(fn, phase); REQUIRE_PTR(fn, iota); REQUIRE_PTR(fn, phi); REQUIRE_PTR(fn, psi);
+  REQUIRE_PTR(fn, lambda); REQUIRE_PTR(fn, beta_sky); REQUIRE_PTR(fn, data_spec); REQUIRE_PTR(fn, weight);
+  REQUIRE_PTR(fn, loglike); REQUIRE_PTR(fn, workspace);
+  const int nang = (alpha != 0) + (beta != 0) + (gamma != 0);
+  if (nang != 0 && nang != 3) return set_error(LISA_TD_EINVAL, "%s: alpha, beta, gamma must be all NULL or all given", fn);
+  OPTIONAL_PTR(fn, alpha); OPTIONAL_PTR(fn, beta); OPTIONAL_PTR(fn, gamma);
+  if ((rc = check_band(fn, N, kmin, kmax))) return rc;
+  if (workspace_bytes < lisa_td_loglike_from_modes_workspace_bytes(B, N))
+    return set_error(LISA_TD_ENOMEM, "%s: workspace of %lld bytes is smaller than the %lld needed", fn, workspace_bytes,
+                     lisa_td_loglike_from_modes_workspace_bytes(B, N));
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
+  if ((rc = check_margin_y(fn, N, dt, order, margin_y, od))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od, margin_y))) return rc;
+  const long long d = (long long)sizeof(double);
+  char* w = static_cast<char*>(workspace);
+  double* hp = reinterpret_cast<double*>(w);
+  double* hc = reinterpret_cast<double*>(w + al256(d * B * N));
+  double* y = reinterpret_cast<double*>(w + 2 * al256(d * B * N));
+  double* tdi = reinterpret_cast<double*>(w + 2 * al256(d * B * N) + al256(d * 6 * B * N));
+  double* tab = reinterpret_cast<double*>(w + 2 * al256(d * B * N) + al256(d * 6 * B * N) + al256(d * 3 * B * N));
+  cudaStream_t st = (cudaStream_t)stream;
+  if ((rc = run_modes_to_pol(B, N, n_modes, l_host, m_host, amp, phase, alpha, beta, gamma, iota, phi, psi, nullptr, hp, hc, st)))
+    return rc;
+  if ((rc = run_link_response(B, N, t0, dt, order, margin_y, hp, hc, lambda, beta_sky, od, y, st))) return rc;
+  if ((rc = run_tdi(B, N, t0, dt, order, generation, 1, margin_lo, margin_hi, y, od, tdi, st, tab, tdi_workspace_bytes(N))))
+    return rc;
+  return run_loglike(plan->p, B, N, tdi, data_spec, weight, kmin, kmax, loglike, dh, hh, st, 3);
+}
+
 int lisa_td_loglike_channels(lisa_td_plan* plan, int B, long long N, int n_channels, const double* tdi,
                              const double* data_spec, const double* weight, long long kmin, long long kmax,
                              double* loglike, double* dh, double* hh, void* stream) {

@@ -25,6 +25,7 @@ EXPORTS = [
     "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
     "lisa_td_pipeline_destroy", "lisa_td_pipeline_host", "lisa_td_pipeline_host_up2", "lisa_td_check",
+    "lisa_td_loglike_from_modes_workspace_bytes", "lisa_td_loglike_from_modes",
 ]
 PROBE_LIB_PATH = os.path.join(_HERE, "liblisa_td_probe.so")  # bench-only, csrc/lisa_td_probe.h
 
@@ -133,6 +134,11 @@ def load() -> C.CDLL:
                                            i64, i64, vp, vp, vp])
     L.lisa_td_pipeline_host_up2.argtypes = L.lisa_td_pipeline_host.argtypes
     L.lisa_td_check.argtypes = [vp]
+    L.lisa_td_loglike_from_modes_workspace_bytes.restype = i64
+    L.lisa_td_loglike_from_modes_workspace_bytes.argtypes = [i32, i64]
+    L.lisa_td_loglike_from_modes.argtypes = ([vp, i32, i64, i32, C.POINTER(i32), C.POINTER(i32)] + [vp] * 10
+                                             + [dbl, dbl, i32, i64, i32, i64, i64, C.POINTER(Orbit), vp, vp, i64, i64,
+                                                vp, vp, vp, vp, i64, vp])
     _lib = L
     return L
 
@@ -264,6 +270,21 @@ def loglike(plan: Plan, B, N, tdi, data_spec, weight, kmin, kmax, loglike_out, d
 def loglike_channels(plan: Plan, B, N, n_channels, tdi, data_spec, weight, kmin, kmax, loglike_out, dh=None, hh=None):
     _check(load().lisa_td_loglike_channels(plan._h, B, N, int(n_channels), _dev(tdi), _dev(data_spec), _dev(weight),
                                            kmin, kmax, _dev(loglike_out), _dev(dh), _dev(hh), _stream()))
+
+
+def loglike_from_modes_workspace_bytes(B, N) -> int:
+    return load().lisa_td_loglike_from_modes_workspace_bytes(B, N)
+
+
+def loglike_from_modes(plan: Plan, B, N, l, m, amp, phase, alpha, beta, gamma, iota, phi, psi, lam, beta_sky, t0, dt,
+                       order, margin_y, generation, margin_lo, margin_hi, orbit, data_spec, weight, kmin, kmax,
+                       loglike_out, dh, hh, workspace):
+    o = make_orbit(orbit)
+    _check(load().lisa_td_loglike_from_modes(
+        plan._h, B, N, len(l), _ints(l), _ints(m), _dev(amp), _dev(phase), _dev(alpha), _dev(beta), _dev(gamma),
+        _dev(iota), _dev(phi), _dev(psi), _dev(lam), _dev(beta_sky), t0, dt, order, margin_y, generation, margin_lo,
+        margin_hi, C.byref(o), _dev(data_spec), _dev(weight), kmin, kmax, _dev(loglike_out), _dev(dh), _dev(hh),
+        _dev(workspace), workspace.numel() * workspace.element_size(), _stream()))
 
 
 def spectrum(plan: Plan, B, N, tdi, spec):

@@ -424,3 +424,43 @@ def test_pipeline_host_matches_stagewise(lib, orc):
     assert np.max(np.abs(out2 - ref["loglike"]) / np.abs(ref["loglike"])) < TOL_LL
     pipe.close()
     plan.close()
+
+
+def test_loglike_from_modes_is_the_stagewise_path_in_one_call(lib, orc):
+    """lisa_td_loglike_from_modes (S1..S5 from device inputs, one call) against the four stage calls (bit for
+    bit: the same kernels in the same order) and against the oracle's own chain."""
+    B, N = 5, 1 << 13
+    inp = synth.make_inputs(4, B=B, N=N)
+    dt = inp["dt"]
+    kmin, kmax = synth.likelihood_band(N, dt)
+    w = orc.psd_weights(N, dt, synth.NOISE["acc"], synth.NOISE["oms"], synth.NOISE["arm_s"], 20)
+    data = orc.spectrum3(_orc_chain(orc, inp, 20, 1, want=("tdi",))["tdi"][0])
+    ref = _orc_chain(orc, inp, 20, 1, want=("loglike",), data_spec=data, weight=w, kmin=kmin, kmax=kmax)
+    d = lambda k: None if inp[k] is None else inp[k].cuda()
+    plan = lib.Plan(B, N)
+    ws = torch.empty(lib.loglike_from_modes_workspace_bytes(B, N) // 8, dtype=torch.float64, device="cuda")
+    ll, dh, hh = (torch.empty(B, dtype=torch.float64, device="cuda") for _ in range(3))
+    lib.loglike_from_modes(plan, B, N, inp["l"], inp["m"], d("amp"), d("phase"), d("alpha"), d("beta"), d("gamma"),
+                           d("iota"), d("phi"), d("psi"), d("lam"), d("beta_sky"), inp["t0"], dt, inp["order"],
+                           inp["margin_y"], 20, inp["margin_lo"], inp["margin_hi"], inp["orbit"], dev(data), dev(w),
+                           kmin, kmax, ll, dh, hh, ws)
+    lib.check()
+    for got, key in ((ll, "loglike"), (dh, "dh"), (hh, "hh")):
+        assert np.max(np.abs(got.cpu().numpy() - ref[key]) / np.abs(ref[key])) < TOL_LL
+    _, _, _, tdi = _gpu_chain(lib, inp, 20, 1)
+    ll2 = torch.empty(B, dtype=torch.float64, device="cuda")
+    lib.loglike(plan, B, N, dev(tdi), dev(data), dev(w), kmin, kmax, ll2)
+    torch.cuda.synchronize()
+    assert torch.equal(ll, ll2)
+    # a workspace that is too small, or TDI margins that do not include margin_y, are rejected before any launch
+    with pytest.raises(lib.LisaTdError):
+        lib.loglike_from_modes(plan, B, N, inp["l"], inp["m"], d("amp"), d("phase"), d("alpha"), d("beta"), d("gamma"),
+                               d("iota"), d("phi"), d("psi"), d("lam"), d("beta_sky"), inp["t0"], dt, inp["order"],
+                               inp["margin_y"], 20, inp["margin_lo"], inp["margin_hi"], inp["orbit"], dev(data), dev(w),
+                               kmin, kmax, ll, dh, hh, ws[:1000])
+    with pytest.raises(lib.LisaTdError):
+        lib.loglike_from_modes(plan, B, N, inp["l"], inp["m"], d("amp"), d("phase"), d("alpha"), d("beta"), d("gamma"),
+                               d("iota"), d("phi"), d("psi"), d("lam"), d("beta_sky"), inp["t0"], dt, inp["order"],
+                               inp["margin_y"], 20, 40, inp["margin_hi"], inp["orbit"], dev(data), dev(w),
+                               kmin, kmax, ll, dh, hh, ws)
+    plan.close()

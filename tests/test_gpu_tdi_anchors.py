@@ -1,9 +1,9 @@
 """GPU parity of the anchored merged-stencil TDI kernel (k3_tdi_mma) where its assumptions end.
 
-The kernel evaluates the merged TDI stencils exactly at three anchor samples per 32-sample tile and
-gives every row the quadratic through them; that is valid only while no integer delay K = ceil(D)
-changes inside the tile and the orbit is one smooth function over it.  Tiles where that fails take an
-exact per-row path.  These tests put such tiles on purpose -- an integer delay crossing in the middle
+The kernel evaluates the merged TDI stencils exactly at three anchor samples per group of 128 samples
+(four 32-sample MMA tiles) and gives every row the quadratic through them; that is valid only while no
+integer delay K = ceil(D) changes inside the group and the orbit is one smooth function over it.  Groups
+where that fails are recomputed sample by sample (k3_tdi_fixup).  These tests put such tiles on purpose -- an integer delay crossing in the middle
 of the grid, a tabulated orbit with a node every 80 samples -- and compare with the long-double
 oracle on WHITE link series (every tap matters: a row served by the wrong window is wrong at O(1)).
 Eq. 2.9-2.11; readings A10, A21, A22 of DESIGN.md.
