@@ -99,9 +99,11 @@ def test_s1_parity(lib, orc, modes, twisted, with_e0, force_generic):
         lib.debug_force_generic(0)
     scale = np.sum(amp, axis=1)
     for g, r in zip(got, ref):
-        # up to l+2 = 10 chained complex products per row and 2 n_modes rows: a few 1e-16 each
-        assert np.max(np.abs(g - r) / scale) < 2e-14
-        assert rel_l2(g, r) < 5e-15
+        # The bars of the first oracle commit, restored: max abs 5e-15 of the summed amplitudes (measured
+        # 1.5e-15) and rel-L2 2e-15 for the paper's mode sets (measured 1.2e-15).  The ten-mode l <= 8 list
+        # chains up to l+2 = 10 complex products per row over 2 n_modes rows: measured 3.0e-15, bar 5e-15.
+        assert np.max(np.abs(g - r) / scale) < 5e-15
+        assert rel_l2(g, r) < (2e-15 if len(modes) <= 5 else 5e-15)
 
 
 @pytest.mark.parametrize("B,N", [(5, 1 << 16), (2, 1026), (3, 2501)])
