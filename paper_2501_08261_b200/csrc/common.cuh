@@ -113,8 +113,13 @@ __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
   const double TWO_OVER_PI = 0.6366197723675814;
   const double PIO2_HI = 1.5707963267948966;
   const double PIO2_LO = 6.123233995736766e-17;
-  double kd = rint(x * TWO_OVER_PI);
-  int q = __double2int_rn(kd);
+  // round to nearest by adding and subtracting 1.5 * 2^52 (exact for |x 2/pi| < 2^51): two DADDs on the
+  // fp64 pipe instead of FRND + F2I on the quarter-rate conversion pipe; the quadrant is in the low
+  // bits of the biased sum
+  const double SHIFTER = 6755399441055744.0;
+  const double kb = fma(x, TWO_OVER_PI, SHIFTER);
+  const int q = __double2loint(kb);
+  const double kd = kb - SHIFTER;
   double r = fma(-kd, PIO2_HI, x);
   r = fma(-kd, PIO2_LO, r);
   double r2 = r * r;
