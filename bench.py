@@ -272,6 +272,20 @@ def run_ours(args):
         pipes[name] = {"ms": pms, "tflops": 2 * 100000 * 148 * (256 * nf_w + 1024 * nm_w) / (pms * 1e-3) / 1e12}
     pipes["reading"] = "times add: one fp64 resource" if pipes["both"]["ms"] > 0.9 * (pipes["dfma_only"]["ms"] + pipes["dmma_only"]["ms"]) else "overlap"
 
+    # issue rate of fp64 instructions by the number of distinct register operands: a DFMA that
+    # reads three fresh registers issues every 3 cycles, not 2; "k2_sweep_only" is the node-pair recurrence of
+    # K2's sweep on register data, i.e. what that instruction mix can reach with no loads at all
+    operands = {}
+    for name, (pat, per_round) in (("fma_1_register_operand", (0, 8)), ("mul_2_register_operands", (1, 8)),
+                                   ("fma_2_fresh_1_repeated", (2, 8)), ("fma_3_register_operands", (3, 8)),
+                                   ("k2_sweep_only", (4, 352))):
+        lib.probe_fp64_operands(pat, 2000, 148 * 4, sink)
+        it_o = 200000 if pat < 4 else 5000
+        oms = lib.probe_fp64_operands(pat, it_o, 148 * 4, sink)
+        operands[name] = {"ms": oms, "tflops_equiv": 2 * per_round * it_o * 148 * 4 * 128 / (oms * 1e-3) / 1e12}
+    for v in operands.values():
+        v["frac_of_dfma_peak"] = v["tflops_equiv"] / dfma_peak_tflops
+
     stages = [("S1_modes_to_pol", s1), ("S2_link_response", s2), ("S3_tdi2", s3), ("S45_fft_loglike", s45)]
     for _ in range(max(args.warmup, 3)):
         for _, fn in stages:
@@ -506,6 +520,10 @@ def run_ours(args):
     # the 0.76 of K2 credits 1725 ops, 98 % of what the kernel executes; the count SURVEY 8(d) priced
     # (576 stencil FMAs + 100 geometry, without the nine walker-dependent coefficient sets) gives:
     roofline["frac_survey_priced_ops"] = 2 * (576 + 100) * ws / (k2_ms * 1e-3) / 1e12 / dfma_peak_tflops
+    # what K2's instruction mix can reach at all: four of the eleven fp64 instructions of a node pair read three
+    # fresh registers and issue every 3 cycles (probe above), so the sweep's own ceiling is ~0.85 of the DFMA peak
+    roofline["operand_probe"] = operands
+    roofline["frac_of_instruction_mix_ceiling"] = roofline["frac"] / operands["k2_sweep_only"]["frac_of_dfma_peak"]
 
     # ---- end to end through the host API (pinned host buffers, copies inside the timed region)
     e2e = None

@@ -45,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
         subprocess.run(cmd, check=True)
     probe_src = os.path.join(CSRC, "probe.cu")
-    if force or _stale(PROBE_LIB, [probe_src, os.path.join(CSRC, "lisa_td_probe.h")]):
+    if force or _stale(PROBE_LIB, [probe_src, os.path.join(CSRC, "lisa_td_probe.h")] + HEADERS):
         subprocess.run([NVCC, *FLAGS, "-shared", probe_src, "-o", PROBE_LIB], check=True)
     return LIB
 

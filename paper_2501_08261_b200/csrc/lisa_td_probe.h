@@ -27,6 +27,18 @@ __attribute__((visibility("default"))) int lisa_td_probe_dfma(long long iters, i
 __attribute__((visibility("default"))) int lisa_td_probe_fp64_pipes(long long iters, int blocks, int dfma_warps,
                                                                     int dmma_warps, double* sink, float* ms_host,
                                                                     void* stream);
+
+/* Issue rate of fp64 instructions by the number of distinct register operands they read, on
+ * `blocks` x 128 threads (4 blocks per SM resident), `iters` rounds:
+ *   pattern 0: a = fma(a, const, const)      8 per round, one register operand
+ *   pattern 1: a = a * b                     8 per round, two register operands
+ *   pattern 2: a = fma(a, b, c0)             8 per round, two fresh + one repeated operand
+ *   pattern 3: a = fma(a, b, c)              8 per round, three distinct register operands
+ *   pattern 4: K2's order-31 Lagrange sweep (lagrange_dot2h_x2<16> of common.cuh) on a shared-memory
+ *              tile in K2's block shape, 352 per round: the ceiling of K2's instruction mix
+ * Instruction count per thread = (pattern < 4 ? 8 : 352) * iters.  sink: blocks * 128 doubles. */
+__attribute__((visibility("default"))) int lisa_td_probe_fp64_operands(int pattern, long long iters, int blocks,
+                                                                       double* sink, float* ms_host, void* stream);
 #ifdef __cplusplus
 }
 #endif

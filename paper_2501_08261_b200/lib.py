@@ -359,6 +359,7 @@ def _probe_lib() -> C.CDLL:
         vp, i32, i64 = C.c_void_p, C.c_int, C.c_longlong
         P.lisa_td_probe_dfma.argtypes = [i64, i32, i32, vp, C.POINTER(C.c_float), vp]
         P.lisa_td_probe_fp64_pipes.argtypes = [i64, i32, i32, i32, vp, C.POINTER(C.c_float), vp]
+        P.lisa_td_probe_fp64_operands.argtypes = [i32, i64, i32, vp, C.POINTER(C.c_float), vp]
         _probe = P
     return _probe
 
@@ -367,6 +368,13 @@ def probe_dfma(iters, blocks, threads, sink) -> float:
     ms = C.c_float()
     if _probe_lib().lisa_td_probe_dfma(iters, blocks, threads, _dev(sink), C.byref(ms), _stream()) != 0:
         raise RuntimeError("lisa_td_probe_dfma failed")
+    return ms.value
+
+
+def probe_fp64_operands(pattern, iters, blocks, sink) -> float:
+    ms = C.c_float(0.0)
+    if _probe_lib().lisa_td_probe_fp64_operands(pattern, iters, blocks, _dev(sink), C.byref(ms), _stream()) != 0:
+        raise RuntimeError("lisa_td_probe_fp64_operands failed")
     return ms.value
 
 
