@@ -287,7 +287,8 @@ __global__ void __launch_bounds__(256) k3_tdi_fixup(const K3Params p, const int*
 // therefore written by a small kernel of their own (k3_anchor_tables: 12 x 3 x WIN doubles and a
 // split flag per tile, 13 KB) into a workspace, and the persistent MMA kernel (one block per SM,
 // walking over tiles) pulls the table of the NEXT tile into shared memory with one bulk TMA copy
-// while the walkers of the current tile stream through the DMMA loop.
+// while the walkers of the current tile stream through the DMMA loop, and forms the next tile's A
+// fragments under the DMMAs of the current tile's last walker chunk.
 constexpr int K3_TS = 32;                     // output samples per tile (four 8-row MMA blocks)
 constexpr int K3_PAIRS = 12;                  // (channel, series) pairs
 constexpr int K3_THREADS = K3_TS * K3_PAIRS;  // 384: warp = (channel, row block)
@@ -516,6 +517,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
   using G = K3Geom<H, WIN>;
   constexpr int LOW = G::LOW, KSTEPS = G::KSTEPS, TW = G::TW, PAD = G::PAD, QS = G::QS;
   constexpr int NWARPS = K3_THREADS / 32;
+  constexpr bool OVERLAP_FILL = G::BLOCKS_PER_SM == 1;  // form the next tile's A fragments under the last chunk's DMMAs
   __shared__ __align__(8) uint64_t ybar[2];    // TMA completion, one per walker-chunk buffer
   __shared__ __align__(8) uint64_t tbar[2];    // TMA completion, one per anchor-table buffer
   extern __shared__ __align__(128) double smem[];
@@ -578,45 +580,54 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
   for (int q = 0; q < 4; ++q) ser[q] = p.pair[ch * 4 + q].series;
   const bool vec = (p.N & 1) == 0;
 
-  if (my_tiles > 0) prefetch(tile_n0(0), 0, 0);
+  // A fragments of (channel ch, row block rb), pair q of tile `it`: KSTEPS values, the quadratic
+  // through the group's three anchors at this lane's row (a flagged group gets meaningless
+  // fragments: the fix-up pass behind this kernel overwrites its outputs)
+  double A[4][KSTEPS];
+  auto fill_pair = [&](const int q, const int it) {
+    const double* src = qtab + (it & 1) * G::QBUF + (ch * 4 + q) * 3 * QS;
+    const double u = (double)((int)(tile_id(it) % K3_GT) * K3_TS + rb * 8 + r) * (1.0 / K3_AH);
+    const double w0 = 0.5 * (u - 1.0) * (u - 2.0), w1 = u * (2.0 - u), w2 = 0.5 * u * (u - 1.0);
+#pragma unroll
+    for (int ks = 0; ks < KSTEPS; ++ks) {
+      const int i = 4 * ks + kk - r;
+      const bool in = i >= 0 && i < WIN;
+      const int ic = in ? i : 0;
+      const double v = fma(w2, src[2 * QS + ic], fma(w1, src[QS + ic], w0 * src[ic]));
+      A[q][ks] = in ? v : 0.0;
+    }
+  };
+
+  if (my_tiles > 0) {
+    prefetch(tile_n0(0), 0, 0);
+    mbar_wait(&tbar[0], 0u);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) fill_pair(q, 0);
+  }
   unsigned g = 0;  // chunks processed so far (y and exchange buffers alternate on it)
   for (int it = 0; it < my_tiles; ++it) {
-    const int tb = it & 1;
     const long long n0 = tile_n0(it);
-    // the table buffer of the next tile was last read by the A fragments of the previous tile,
-    // which every warp completed before the barriers of that tile's chunks
-    if (threadIdx.x == 0 && it + 1 < my_tiles) fetch_table(it + 1);
-    mbar_wait(&tbar[tb], (unsigned)((it >> 1) & 1));
-    // ---- A fragments of (channel ch, row block rb): 4 pairs x KSTEPS values
-    const double* qt = qtab + tb * G::QBUF;
-    // (a tile whose table carries the split flag gets meaningless fragments here: the fix-up pass
-    // behind this kernel overwrites its outputs)
-    double A[4][KSTEPS];
-    {
-      // weights of the three anchors at this lane's row (quadratic through samples 0, 64, 128 of the group)
-      const double u = (double)((int)(tile_id(it) % K3_GT) * K3_TS + rb * 8 + r) * (1.0 / K3_AH);
-      const double w0 = 0.5 * (u - 1.0) * (u - 2.0), w1 = u * (2.0 - u), w2 = 0.5 * u * (u - 1.0);
+    const bool have_next = it + 1 < my_tiles;
+    // the table buffer of the next tile was last read when the fragments of tile it - 1 ... were
+    // formed, i.e. before the barriers of the chunks behind us
+    if (threadIdx.x == 0 && have_next) fetch_table(it + 1);
+    if (!OVERLAP_FILL && it > 0) {  // short stencils (order 1, two blocks per SM): the fill is a few loads, up front
+      mbar_wait(&tbar[it & 1], (unsigned)((it >> 1) & 1));
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const double* src = qt + (ch * 4 + q) * 3 * QS;
-#pragma unroll
-        for (int ks = 0; ks < KSTEPS; ++ks) {
-          const int i = 4 * ks + kk - r;
-          const bool in = i >= 0 && i < WIN;
-          const int ic = in ? i : 0;
-          const double v = fma(w2, src[2 * QS + ic], fma(w1, src[QS + ic], w0 * src[ic]));
-          A[q][ks] = in ? v : 0.0;
-        }
-      }
+      for (int q = 0; q < 4; ++q) fill_pair(q, it);
     }
 
-    // ---- stream the walkers
+    // ---- stream the walkers.  In the LAST chunk of a tile the fragments of the NEXT tile are formed
+    // pair by pair, each as soon as the DMMAs of that pair have been issued: its 39 shared-memory
+    // loads and FMAs run under the DMMAs of the following pairs (and of the other warps) instead of
+    // in a phase of their own in which the tensor path idles.
     for (int c = 0; c < n_chunks; ++c, ++g) {
       const int buf = g & 1;
+      const bool refill = OVERLAP_FILL && have_next && c == n_chunks - 1;
       // the other y buffer was last read in the previous chunk, which every MMA warp has left
       bool more = true;
       if (c + 1 < n_chunks) prefetch(n0, c + 1, buf ^ 1);
-      else if (it + 1 < my_tiles) prefetch(tile_n0(it + 1), 0, buf ^ 1);
+      else if (have_next) prefetch(tile_n0(it + 1), 0, buf ^ 1);
       else more = false;
       if (use_tma) {
         mbar_wait(&ybar[buf], (g >> 1) & 1);
@@ -625,6 +636,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
         else cp_async_wait<0>();
         __syncthreads();  // cp.async path: other threads' copies become visible here
       }
+      if (refill) mbar_wait(&tbar[(it + 1) & 1], (unsigned)(((it + 1) >> 1) & 1));
       double* xsc = xs + (size_t)buf * (3 * K3_TS * K3_XS);
       // lane's B element: walker (r | r + 8) of the chunk, time rb*8 + 4 ks + kk
       const double* yb = ys + (size_t)buf * G::YBUF + (size_t)r * 6 * TW + rb * 8 + kk + PAD;
@@ -645,6 +657,7 @@ __global__ void __launch_bounds__(K3_THREADS, K3Geom<H, WIN>::BLOCKS_PER_SM)
             dmma884(e10, e11, A[q][ks], y1[4 * ks]);
           }
         }
+        if (refill) fill_pair(q, it + 1);
       }
       d00 += e00; d01 += e01; d10 += e10; d11 += e11;
       {
@@ -740,9 +753,9 @@ static int launch_mma(const K3Params& p, double* tab, cudaStream_t st) {
   k3_anchor_tables<H, WIN><<<(unsigned)((n_groups + K3_TAB_TILES - 1) / K3_TAB_TILES), K3_TAB_THREADS, 0, st>>>(p, tab, list, (int)n_groups);
   LISA_LAUNCH_CHECK("k3_anchor_tables");
   // 2. persistent MMA blocks: one (two at order 1) per SM, each walking over tiles blockIdx.x + i gridDim.x
-  LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
   const long long resident = (long long)G::BLOCKS_PER_SM * sm_count();
   const unsigned grid = (unsigned)(n_tiles < resident ? n_tiles : resident);
+  LISA_CUDA(cudaFuncSetAttribute(k3_tdi_mma<H, WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
   k3_tdi_mma<H, WIN><<<grid, K3_THREADS, G::SMEM, st>>>(p, tmap, use_tma, tab, (int)n_tiles);
   LISA_LAUNCH_CHECK("k3_tdi_mma");
   // 3. fix-up: the flagged tiles, sample by sample (threads of other tiles leave at once)
