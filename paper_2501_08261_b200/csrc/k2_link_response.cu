@@ -48,6 +48,17 @@ __device__ __forceinline__ void k2_cp_async8_zfill(void* smem, const void* gmem,
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(sa), "l"(gmem), "r"(sz));
 }
 
+// 1/x for the geometric factors 1/((1 - k.n_A)(1 - k.n_B)), x in (0, 4]: the hardware seed (MUFU.RCP64H,
+// ~23 bits) and two Newton steps, good to one ulp -- a third of the instructions of the IEEE-exact
+// division, whose slow-path test and call sit six times in every walker's loop body.
+__device__ __forceinline__ double k2_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  r = fma(fma(-x, r, 1.0), r, r);
+  r = fma(fma(-x, r, 1.0), r, r);
+  return r;
+}
+
 // Fractional-delay reads of (h+, hx) for the sample pair (a, b = a+1) at delays
 // D = Dc + Dl (samples).  The integer part is decided from the rounded sum, the fraction is
 // formed as (K - Dc) - Dl so that the common 1 AU part (up to ~100 samples) does not cost the
@@ -268,7 +279,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response(const K2Params
               xpB[c] = fma(unB, unB, -vnB * vnB);
               xcB[c] = 2.0 * unB * vnB;
               const double omA = 1.0 - keA * ilAs[c], omB = 1.0 - keB * ilBs[c];  // 1 - k.n of each link
-              const double inv = 0.5 / (omA * omB);
+              const double inv = 0.5 * k2_rcp(omA * omB);
               fA[c] = omB * inv;
               fB[c] = omA * inv;
             }
@@ -410,7 +421,7 @@ __global__ void __launch_bounds__(K2_THREADS, 4) k2_link_response_lin(const K2Pa
         xp[c] = fma(un, un, -vn * vn);
         xc2[c] = 2.0 * un * vn;
         const double om = 1.0 - kn, opl = 1.0 + kn;
-        const double inv = 0.5 / (om * opl);
+        const double inv = 0.5 * k2_rcp(om * opl);
         fp[c] = opl * inv;
         fm[c] = om * inv;
       }
