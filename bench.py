@@ -47,7 +47,7 @@ K2_GEOM = 150
 K2_OPS = K2_SWEEP + K2_GEOM            # 1725 ops = 3450 flop per walker-sample
 K2_BYTES = 16 + 48                     # h+,hx in, six links out
 # dram__bytes_read.sum + dram__bytes_write.sum of one k2 launch at this workload
-# (ncu --set full capture summarised in profiles/r2_s1.md: 1.07 GB read + 3.17 GB written)
+# (ncu --set full capture summarised in profiles/r2_s2.md: 1.08 GB read + 3.17 GB written)
 K2_TRAFFIC_BYTES = 4.24e9
 # K3 (TDI-2, A,E,T): 12 (channel, series) pairs x 44 merged-stencil taps = 528 MACs per walker-sample
 # (the 8x8x4 tiles of the banded product issue 624); 48 B of links in, 24 B out
