@@ -99,6 +99,18 @@ def test_probes_and_debug_switches_are_not_part_of_the_abi(lib):
     assert not hasattr(L, "lisa_td_probe_dfma") and not hasattr(L, "lisa_td_debug_force_generic")
 
 
+def test_probe_library_exports_what_its_header_declares(lib):
+    """the bench-only probe library (csrc/lisa_td_probe.h) loads without a GPU and exports every
+    entry point its header declares; bench.py's roofline denominators come from these"""
+    import re
+    hdr = open(os.path.join(ROOT, "paper_2501_08261_b200", "csrc", "lisa_td_probe.h")).read()
+    declared = sorted(set(re.findall(r"\b(lisa_td_probe_\w+)\s*\(", hdr)))
+    assert declared == ["lisa_td_probe_dfma", "lisa_td_probe_fp64_operands", "lisa_td_probe_fp64_pipes"]
+    P = lib._probe_lib()
+    for name in declared:
+        assert hasattr(P, name), name
+
+
 def test_psd_weights_host_helper_matches_oracle(lib, orc):
     """the CUDA library's host helper against the oracle's (pinned in test_oracle_psd_transfer.py),
     EVERY bin, with a tolerance that follows the conditioning of Eq. 2.15: w ~ 1 / (sin^2 x sin^2 2x ...),
