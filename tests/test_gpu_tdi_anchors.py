@@ -105,10 +105,12 @@ def test_anchored_rows_match_the_generic_kernel(lib):
     assert np.max(np.abs(a - b)) < 2e-14 * np.sqrt(np.mean(b ** 2)) * 10
 
 
-@pytest.mark.parametrize("N,B", [(70, 1), (130, 2), (257, 17), (1000, 16), (1153, 40)])
+@pytest.mark.parametrize("N,B", [(70, 1), (130, 2), (257, 17), (1000, 16), (1153, 40), (6002, 40), (9000, 17)])
 def test_short_and_ragged_grids(lib, orc, N, B):
     """fewer samples than one anchor group (128) or one MMA tile (32), odd N (cp.async path), grids that
-    end inside a group, walker counts around the chunk size of 16"""
+    end inside a group, walker counts around the chunk size of 16; the two long grids give a persistent
+    block more than one tile (148 blocks, 188 and 282 tiles), so the A fragments of the next tile are formed
+    under the last -- ragged -- walker chunk of the current one"""
     rng = np.random.default_rng(N + B)
     dt, order, t0 = 5.0, 31, 5.0e6
     orbit = synth.kepler_orbit()
