@@ -173,6 +173,25 @@ LISA_TD_API int lisa_td_tdi2(int B, long long N, double t0, double dt, int order
                  long long margin_lo, long long margin_hi, const double* y,
                  const lisa_td_orbit* orbit_host, double* tdi, void* stream);
 
+/* S3 without any allocation -- lisa_td_tdi2 (same arguments, same kernels, same output) for callers
+ * that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it.  The merged-stencil tables and the fix-up list that lisa_td_tdi2 draws from the memory
+ * pool live in ONE file-scope device array of the library instead (about 7 MiB, held by every GPU
+ * that loads the library until the process exits), sized for N <= LISA_TD_TDI2_STATIC_MAX_N samples;
+ * a larger N is rejected with LISA_TD_EINVAL before anything is launched.  The call makes no
+ * cudaMalloc / cudaFree / cudaMallocAsync and no allocating library call; the first call on each
+ * device looks the array's address up (cudaGetSymbolAddress), so make that call before capturing.
+ * Every call shares the array: it clears what must start at zero itself, and two calls that overlap
+ * on the GPU (different streams without an ordering between them, or two host threads) RACE.
+ * Device-side range checks of this entry point are kept in the array too, not in the words
+ * lisa_td_check reads: check != 0 makes the call wait for `stream` and return LISA_TD_EINVAL if a
+ * stencil left its window in this call or in an earlier call with check == 0 (then cleared);
+ * check == 0 only enqueues (use this under capture). */
+#define LISA_TD_TDI2_STATIC_MAX_N 65536
+LISA_TD_API int lisa_td_tdi2_static(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+                 long long margin_lo, long long margin_hi, const double* y,
+                 const lisa_td_orbit* orbit_host, double* tdi, int check, void* stream);
+
 /* S2+S3 in one call: h+,hx -> tdi.  This is lisa_td_link_response into `workspace` followed by
  * lisa_td_tdi2 from it: all six links of all B walkers make one round trip through HBM ([B][6][N]
  * doubles = 48 B N bytes; lisa_td_response_tdi_workspace_bytes returns that plus the anchor

@@ -285,6 +285,8 @@ int run_laser_links(long long, double, double, int, long long, const double*, co
 int run_tdi(int, long long, double, double, int, int, int, long long, long long, const double*,
             const OrbitDev&, double*, cudaStream_t, double* tab_ws = nullptr, long long tab_ws_bytes = 0);
 long long tdi_workspace_bytes(long long N);
+int run_tdi_static(int, long long, double, double, int, int, int, long long, long long, const double*,
+                   const OrbitDev&, double*, int check, cudaStream_t);
 struct Plan;
 int plan_create(Plan**, int, long long);
 int plan_destroy(Plan*);
@@ -498,6 +500,26 @@ int lisa_td_tdi2(int B, long long N, double t0, double dt, int order, int genera
   if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
   return run_tdi(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi,
                  (cudaStream_t)stream);
+}
+
+// lisa_td_tdi2 with its scratch in a file-scope device array (k3_tdi.cu): no allocation of any kind
+int lisa_td_tdi2_static(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+                        long long margin_lo, long long margin_hi, const double* y,
+                        const lisa_td_orbit* orbit_host, double* tdi, int check, void* stream) {
+  const char* fn = "lisa_td_tdi2_static";
+  int rc = check_common(fn, B, N, dt, order);
+  if (rc) return rc;
+  if (N > LISA_TD_TDI2_STATIC_MAX_N)
+    return set_error(LISA_TD_EINVAL, "%s: N=%lld exceeds LISA_TD_TDI2_STATIC_MAX_N=%d samples (the size of the static scratch array)",
+                     fn, N, LISA_TD_TDI2_STATIC_MAX_N);
+  if (out_kind != 0 && out_kind != 1) return set_error(LISA_TD_EINVAL, "%s: out_kind must be 0 (XYZ) or 1 (AET)", fn);
+  REQUIRE_PTR(fn, y); REQUIRE_PTR(fn, tdi);
+  OrbitDev od;
+  if ((rc = make_orbit_dev(orbit_host, &od))) return rc;
+  if ((rc = check_table_range(fn, orbit_host, N, t0, dt))) return rc;
+  if ((rc = check_margin_tdi(fn, N, dt, order, generation, margin_lo, margin_hi, od))) return rc;
+  return run_tdi_static(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, od, tdi, check,
+                        (cudaStream_t)stream);
 }
 
 // [B][6][N] link responses, then the anchor tables of S3 (k3_tdi.cu)

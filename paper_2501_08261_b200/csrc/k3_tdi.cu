@@ -825,4 +825,106 @@ int run_tdi(int B, long long N, double t0, double dt, int order, int generation,
   return LISA_TD_OK;
 }
 
+// ---------------------------------------------------------------- no-allocation variant (lisa_td_tdi2_static)
+// Same kernels as run_tdi; the anchor tables and the fix-up list live in a file-scope device array
+// instead of a stream-ordered temporary, so the call allocates nothing (callers under CUDA graph
+// capture, serving loops or harnesses that forbid cudaMalloc).  Every GPU that loads the library
+// holds the array until exit; it is sized for K3_STATIC_MAX_N samples.  Layout:
+//   [0, 256)   header: DEVERR_COUNT sticky error words of THIS entry point (device memory; the
+//              other entry points use mapped host words, common.cuh, whose first use allocates)
+//   [256, ...) anchor tables [groups][12][3][QS] and the list of flagged groups, as tdi_workspace_bytes
+// The array keeps the last call's contents: the list count is cleared by every call
+// (launch_mma), the tables of the groups a call uses are rewritten by it, the error words stay
+// set until a call with check != 0 reads and clears them.  Calls that overlap on the GPU race.
+constexpr long long K3_STATIC_MAX_N = LISA_TD_TDI2_STATIC_MAX_N;
+constexpr long long K3_STATIC_GROUPS = (K3_STATIC_MAX_N + K3_GS - 1) / K3_GS;
+constexpr size_t k3_round256(size_t b) { return (b + 255) / 256 * 256; }
+constexpr size_t K3_STATIC_HDR = 256;
+constexpr size_t K3_STATIC_BYTES = K3_STATIC_HDR + k3_round256((size_t)K3_STATIC_GROUPS * K3Geom<16, 48>::QBUF * sizeof(double)) +
+                                   k3_round256((size_t)(K3_STATIC_GROUPS + 1) * sizeof(int));
+static_assert(K3_STATIC_BYTES <= (size_t)8 << 20, "the static scratch is meant to stay modest (8 MiB)");
+static_assert(DEVERR_COUNT * sizeof(unsigned int) <= K3_STATIC_HDR, "header holds the error words");
+static __device__ __align__(256) unsigned char k3_static_scratch[K3_STATIC_BYTES];
+
+// Device address of the array on the CURRENT device.  In host code `k3_static_scratch` is only a
+// handle for the runtime, not a device pointer: the address is looked up once per device.
+static int k3_static_base(unsigned char** out) {
+  constexpr int MAX_DEV = 64;
+  static thread_local unsigned char* addr[MAX_DEV] = {nullptr};
+  int dev = 0;
+  LISA_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= MAX_DEV) return set_error(LISA_TD_EINVAL, "tdi2_static: device ordinal %d not supported", dev);
+  if (!addr[dev]) {
+    void* ptr = nullptr;
+    LISA_CUDA(cudaGetSymbolAddress(&ptr, k3_static_scratch));
+    if (!ptr) return set_error(LISA_TD_ECUDA, "tdi2_static: cudaGetSymbolAddress returned a null address");
+    addr[dev] = static_cast<unsigned char*>(ptr);
+  }
+  *out = addr[dev];
+  return LISA_TD_OK;
+}
+
+int run_tdi_static(int B, long long N, double t0, double dt, int order, int generation, int out_kind,
+                   long long margin_lo, long long margin_hi, const double* y, const OrbitDev& orb,
+                   double* tdi, int check, cudaStream_t st) {
+  if (N > K3_STATIC_MAX_N)
+    return set_error(LISA_TD_EINVAL,
+                     "lisa_td_tdi2_static: N=%lld exceeds LISA_TD_TDI2_STATIC_MAX_N=%lld samples (the size of the static "
+                     "scratch array); use lisa_td_tdi2 or lisa_td_response_tdi with a workspace",
+                     N, K3_STATIC_MAX_N);
+  if (tdi_workspace_bytes(N) > (long long)(K3_STATIC_BYTES - K3_STATIC_HDR))
+    return set_error(LISA_TD_ENOMEM, "lisa_td_tdi2_static: internal: static scratch smaller than the workspace of N=%lld", N);
+  unsigned char* base = nullptr;
+  int rc = k3_static_base(&base);
+  if (rc != LISA_TD_OK) return rc;
+  unsigned int* err = reinterpret_cast<unsigned int*>(base);
+  double* tab = reinterpret_cast<double*>(base + K3_STATIC_HDR);
+  const long long tab_bytes = (long long)(K3_STATIC_BYTES - K3_STATIC_HDR);
+
+  K3Params p;
+  p.B = B; p.N = N; p.t0 = t0; p.dt = dt; p.inv_dt = 1.0 / dt;
+  p.half = (order + 1) / 2; p.generation = generation; p.out_kind = out_kind;
+  p.margin_lo = margin_lo; p.margin_hi = margin_hi; p.y = y; p.tdi = tdi; p.orb = orb;
+  p.err = err;
+  make_lagw(order, &p.lw);
+  make_lags(order, &p.ls);
+  if (build_pairs(generation, p.pair, p.path))
+    return set_error(LISA_TD_EINVAL, "tdi: internal term table does not match the light paths");
+  const int nL = generation == 20 ? 7 : 3;
+  const int kcap = (int)ceil(nL * orb.max_L / dt);
+  p.kcap = kcap;
+  const int need = kcap + 2 * p.half;
+  // run_mma with a workspace argument only launches (no cudaMallocAsync / cudaFreeAsync)
+  bool done = false;
+  if (dispatch_mode() != 1) {
+    if (p.half == 16) {
+      if (need <= 40) { rc = run_mma<16, 40>(p, tab, tab_bytes, st); done = true; }
+      else if (need <= 44) { rc = run_mma<16, 44>(p, tab, tab_bytes, st); done = true; }
+      else if (need <= 48) { rc = run_mma<16, 48>(p, tab, tab_bytes, st); done = true; }
+    } else if (p.half == 1) {
+      if (need <= 8) { rc = run_mma<1, 8>(p, tab, tab_bytes, st); done = true; }
+      else if (need <= 16) { rc = run_mma<1, 16>(p, tab, tab_bytes, st); done = true; }
+    }
+  }
+  if (!done) {  // other orders: one thread per sample, no scratch at all
+    dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);
+    k3_tdi_generic<<<grid, 256, 0, st>>>(p);
+    rc = check_cuda(cudaPeekAtLastError(), "k3_tdi_generic");
+  }
+  if (rc != LISA_TD_OK || !check) return rc;
+  // check != 0: wait for the stream and report the sticky device-side range checks of this entry point
+  unsigned int words[DEVERR_COUNT] = {0};
+  LISA_CUDA(cudaMemcpyAsync(words, err, sizeof(words), cudaMemcpyDeviceToHost, st));
+  LISA_CUDA(cudaStreamSynchronize(st));
+  bool any = false;
+  for (int i = 0; i < DEVERR_COUNT; ++i) any = any || words[i] != 0;
+  if (any) {
+    LISA_CUDA(cudaMemsetAsync(err, 0, sizeof(words), st));
+    return set_error(LISA_TD_EINVAL,
+                     "lisa_td_tdi2_static: a merged TDI stencil left its window on the device (the orbit exceeds the bounds "
+                     "the margins were checked against); the output of this or an earlier unchecked call is wrong");
+  }
+  return LISA_TD_OK;
+}
+
 }  // namespace lisa

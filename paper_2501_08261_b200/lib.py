@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "liblisa_td.so")
 EXPORTS = [
     "lisa_td_last_error", "lisa_td_version", "lisa_td_orbit_table_create", "lisa_td_orbit_table_destroy", "lisa_td_modes_to_pol", "lisa_td_link_response",
     "lisa_td_link_response_up2",
-    "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_response_tdi_workspace_bytes",
+    "lisa_td_laser_links", "lisa_td_tdi2", "lisa_td_tdi2_static", "lisa_td_response_tdi_workspace_bytes",
     "lisa_td_response_tdi", "lisa_td_plan_create", "lisa_td_plan_destroy", "lisa_td_loglike",
     "lisa_td_loglike_channels",
     "lisa_td_spectrum", "lisa_td_fisher", "lisa_td_psd_weights", "lisa_td_pipeline_create",
@@ -116,6 +116,8 @@ def load() -> C.CDLL:
     L.lisa_td_laser_links.argtypes = [i64, dbl, dbl, i32, i64, vp, C.POINTER(Orbit), vp, vp]
     L.lisa_td_tdi2.argtypes = [i32, i64, dbl, dbl, i32, i32, i32, i64, i64, vp, C.POINTER(Orbit),
                                vp, vp]
+    L.lisa_td_tdi2_static.argtypes = [i32, i64, dbl, dbl, i32, i32, i32, i64, i64, vp, C.POINTER(Orbit),
+                                      vp, i32, vp]
     L.lisa_td_response_tdi_workspace_bytes.restype = i64
     L.lisa_td_response_tdi_workspace_bytes.argtypes = [i32, i64]
     L.lisa_td_response_tdi.argtypes = [i32, i64, dbl, dbl, i32, i64, i32, i32, i64, i64, vp, vp, vp,
@@ -227,6 +229,16 @@ def tdi2(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, orb
     o = make_orbit(orbit)
     _check(load().lisa_td_tdi2(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi,
                                _dev(y), C.byref(o), _dev(tdi), _stream()))
+
+
+TDI2_STATIC_MAX_N = 65536  # LISA_TD_TDI2_STATIC_MAX_N of include/lisa_td.h
+
+
+def tdi2_static(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi, y, orbit, tdi, check=True):
+    """lisa_td_tdi2 with its scratch in the library's static device array: allocates nothing, N <= TDI2_STATIC_MAX_N"""
+    o = make_orbit(orbit)
+    _check(load().lisa_td_tdi2_static(B, N, t0, dt, order, generation, out_kind, margin_lo, margin_hi,
+                                      _dev(y), C.byref(o), _dev(tdi), 1 if check else 0, _stream()))
 
 
 def response_tdi_workspace_bytes(B, N) -> int:
